@@ -1,0 +1,207 @@
+"""Pins for the oracle's solvers (Alg. 1, 2, 3 of PAPER.md) against what the
+mathematics fixes (north_star (a)-(d); SURVEY.md §8c "Whole solver"):
+ (a) tiny spd systems converge in <= n iterations to the dense-LU solution;
+ (b) s-step iterate i equals CG iterate i*s;
+ (c) conjugacy -- see test_oracle_kernels.test_one_step_invariants;
+ (d) the closed-form spectrum of the Poisson stencil bounds the A-norm error
+     and the iteration count;
+ (e) Alg. 3 at s=1 == Alg. 2 == Alg. 1 iterates;  (f) Gram form == moment form;
+ (g) the paper's own 514 iterations;  (h) scipy's CG.
+"""
+import os
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import scipy.sparse.linalg as spla
+
+import sstep_inputs as gen
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def csr_of(c):
+    return sp.csr_matrix((c["vals"], c["colidx"], c["rowptr"]), shape=(c["n"], c["n"]))
+
+
+def tiny_systems():
+    out = []
+    rp, ci, v, A = gen.random_spd_csr(48, 0.15, 21)
+    out.append(("rand48", rp, ci, v, A))
+    rp, ci, v = gen.poisson1d(64)
+    out.append(("lap1d64", rp, ci, v, sp.csr_matrix((v, ci, rp)).toarray()))
+    rp, ci, v = gen.poisson7(4)
+    out.append(("p7_4", rp, ci, v, sp.csr_matrix((v, ci, rp)).toarray()))
+    return out
+
+
+# (a) ------------------------------------------------------------------------
+@pytest.mark.parametrize("name,rp,ci,v,A", tiny_systems(), ids=lambda t: t if isinstance(t, str) else "")
+def test_tiny_spd_converges_to_lu(oracle_mod, name, rp, ci, v, A):
+    n = A.shape[0]
+    b = np.random.default_rng(22).uniform(-1, 1, n)
+    xlu = np.linalg.solve(A, b)
+    runs = [("pcg", oracle_mod.pcg(rp, ci, v, b, rtol=1e-11, maxit=n), 1),
+            ("pfcg", oracle_mod.pfcg(rp, ci, v, b, rtol=1e-11, maxit=n), 1)]
+    # s-step: when s does not divide the grade of b the last block [R_1..R_s] is rank deficient and W is
+    # singular (exact breakdown, see test_rank_deficient_last_block); take s | 64 there.
+    for s in ((1, 2, 3, 4) if name == "rand48" else (1, 2, 4)):
+        for form in ("gram", "moment"):
+            runs.append((f"s{s}{form}", oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-9, maxit=-(-n // s) + 2, form=form), s))
+    for tag, res, s in runs:
+        assert res["status"] == 0, (tag, res["relres"])
+        assert res["iters"] * s <= n + 2 * s, tag                         # CG terminates in <= n steps (+ fp64 slack)
+        assert np.linalg.norm(res["x"] - xlu) <= 1e-8 * np.linalg.norm(xlu), tag
+
+
+def test_rank_deficient_last_block(oracle_mod):
+    """Degenerate case of the method: 1-D Laplacian n=64 has grade 64 = 21*3 + 1, so at s=3 the 22nd block
+    spans one new dimension only, W = P^T A P is singular and the Cholesky solve must report breakdown
+    (status 2) instead of returning garbage; x stays the last good iterate."""
+    rp, ci, v = gen.poisson1d(64)
+    b = np.random.default_rng(22).uniform(-1, 1, 64)
+    res = oracle_mod.sstep(rp, ci, v, b, 3, rtol=1e-11, maxit=30)
+    assert res["status"] == 2 and res["iters"] == 21 and np.all(np.isfinite(res["x"]))
+    A = sp.csr_matrix((v, ci, rp)).toarray()
+    assert np.linalg.norm(b - A @ res["x"]) <= 1e-2 * np.linalg.norm(b)
+
+
+def test_lap1d_takes_exactly_n_steps(oracle_mod):
+    """1-D Laplacian, n distinct eigenvalues, generic b: CG needs all n steps."""
+    rp, ci, v = gen.poisson1d(32)
+    b = np.random.default_rng(23).uniform(-1, 1, 32)
+    assert oracle_mod.pcg(rp, ci, v, b, rtol=1e-9, maxit=100)["iters"] == 32
+
+
+# (b), (e), (f) ---------------------------------------------------------------
+def _problems_b():
+    c7 = gen.make_config(1, N=8)
+    c27 = gen.make_config(3, N=6)
+    c5 = gen.make_config(5, N=6)
+    return [c7, c27, c5]
+
+
+@pytest.mark.parametrize("c", _problems_b(), ids=lambda c: c["name"])
+@pytest.mark.parametrize("s", [1, 2, 3, 4])
+def test_sstep_iterates_equal_cg_every_s_steps(oracle_mod, c, s):
+    nouter = 5
+    ref = oracle_mod.pcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=0.0, maxit=nouter * s, xhist_cap=nouter * s)
+    ref2 = oracle_mod.pfcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=0.0, maxit=nouter * s, xhist_cap=nouter * s)
+    scale = np.linalg.norm(ref["xhist"][-1])
+    assert np.abs(ref["xhist"] - ref2["xhist"]).max() <= 1e-13 * scale          # Alg. 1 == Alg. 2
+    for form in ("gram", "moment"):
+        res = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=0.0, maxit=nouter, form=form,
+                               xhist_cap=nouter)
+        assert res["status"] == 1 and res["iters"] == nouter
+        for i in range(nouter):
+            err = np.linalg.norm(res["xhist"][i] - ref["xhist"][(i + 1) * s - 1])
+            assert err <= 5e-11 * scale, (form, s, i, err / scale)
+        if s == 1:
+            assert np.abs(res["xhist"] - ref["xhist"]).max() <= 1e-13 * scale    # (e)
+
+
+@pytest.mark.parametrize("s", [2, 4, 8])
+def test_chebyshev_basis_same_krylov_iterates(oracle_mod, s):
+    """The Gram form is basis-agnostic: the Chebyshev MPK spans the same Krylov
+    space, so iterates still equal CG's every s steps (DESIGN.md NEXT-1)."""
+    c = gen.make_config(1, N=8)
+    nouter = 3
+    ref = oracle_mod.pcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=0.0, maxit=nouter * s, xhist_cap=nouter * s)
+    res = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=0.0, maxit=nouter, basis=1,
+                           xhist_cap=nouter)
+    scale = np.linalg.norm(ref["xhist"][-1])
+    for i in range(nouter):
+        assert np.linalg.norm(res["xhist"][i] - ref["xhist"][(i + 1) * s - 1]) <= 1e-9 * scale
+
+
+def test_composed_steps_equal_driver(oracle_mod):
+    """The C driver orc_sstep is exactly the composition of the per-step functions the parity tests use."""
+    c = gen.make_config(2, N=7)
+    s, nouter = 3, 4
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    dinv = oracle_mod.dinv(rp, ci, v)
+    n = c["n"]
+    x = np.zeros(n); r = b.copy(); P = np.zeros((s, n)); AP = np.zeros((s, n)); W = np.eye(s)
+    for k in range(nouter):
+        R, AR = oracle_mod.mpk(rp, ci, v, dinv, r, s)
+        M, C, m = oracle_mod.gram(R, AR, AP if k else None, r)
+        st, beta, alpha, W = oracle_mod.small_solve(M, C, m, W, first=(k == 0))
+        P, AP, x, r = oracle_mod.update(R, AR, P, AP, x, r, beta, alpha)
+    res = oracle_mod.sstep(rp, ci, v, b, s, rtol=0.0, maxit=nouter)
+    assert np.array_equal(res["x"], x)
+    assert np.isclose(res["relres"], np.linalg.norm(r) / np.linalg.norm(b), rtol=1e-14)
+
+
+# (d) -------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [8, 14])
+def test_cg_error_bound_from_closed_form_spectrum(oracle_mod, N):
+    """||x_k - x*||_A <= 2 ((sqrt(kappa)-1)/(sqrt(kappa)+1))^k ||x_0 - x*||_A with
+    kappa = cot^2(pi / (2(N+1))) for the 7-point stencil (constant diagonal, so
+    Jacobi does not change kappa); and the residual-based iteration count bound."""
+    c = gen.make_config(1, N=N)
+    A = csr_of(c)
+    xs = c["xstar"]
+    kappa = 1.0 / np.tan(np.pi / (2 * (N + 1))) ** 2
+    q = (np.sqrt(kappa) - 1) / (np.sqrt(kappa) + 1)
+    e0 = np.sqrt(xs @ (A @ xs))
+    rtol = 1e-8
+    res = oracle_mod.pcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=rtol, maxit=500, xhist_cap=500, history=True)
+    assert res["status"] == 0
+    for k, xk in enumerate(res["xhist"]):
+        e = xk - xs
+        assert np.sqrt(e @ (A @ e)) <= 2 * q ** (k + 1) * e0 * (1 + 1e-10)
+    # ||r_k||_2 <= sqrt(lmax) ||e_k||_A <= sqrt(kappa) 2 q^k ||r_0||_2  =>  k_stop <= first k with 2 sqrt(kappa) q^k < rtol
+    kbound = int(np.ceil(np.log(rtol / (2 * np.sqrt(kappa))) / np.log(q)))
+    assert res["iters"] <= kbound
+    for s in (2, 4):
+        rs = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=rtol, maxit=500, xhist_cap=500)
+        assert rs["status"] == 0 and rs["iters"] == -(-res["iters"] // s)        # ceil(PCG / s)
+        for i, xi in enumerate(rs["xhist"]):
+            e = xi - xs
+            assert np.sqrt(e @ (A @ e)) <= 2 * q ** ((i + 1) * s) * e0 * (1 + 1e-8)
+
+
+# (h) -------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,N", [(1, 10), (3, 7), (5, 7)])
+def test_pcg_matches_scipy_cg(oracle_mod, cfg, N):
+    c = gen.make_config(cfg, N=N)
+    A = csr_of(c)
+    dinv = 1.0 / A.diagonal()
+    its = []
+    xs, info = spla.cg(A, c["b"], rtol=1e-8, atol=0.0, M=sp.diags(dinv), callback=lambda xk: its.append(xk.copy()))
+    assert info == 0
+    res = oracle_mod.pcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=1e-8, maxit=1000, xhist_cap=len(its) + 5)
+    assert abs(res["iters"] - len(its)) <= 1          # scipy stops on <=, the paper on <
+    k = min(10, len(its), res["iters"])
+    scale = np.linalg.norm(its[k - 1])
+    for i in range(k):
+        assert np.linalg.norm(res["xhist"][i] - its[i]) <= 1e-12 * scale
+    assert np.linalg.norm(res["x"] - xs) <= 1e-7 * np.linalg.norm(xs)
+
+
+def test_status_codes(oracle_mod):
+    c = gen.make_config(1, N=6)
+    args = (c["rowptr"], c["colidx"], c["vals"], c["b"])
+    assert oracle_mod.sstep(*args, 2, rtol=1e-12, maxit=2)["status"] == 1          # maxit
+    r = oracle_mod.sstep(*args, 2, rtol=1e-8, maxit=200, x0=c["xstar"])
+    # x0 already the solution up to rounding: r0 is rounding noise, the relative test still terminates, x stays put
+    assert r["status"] == 0 and np.linalg.norm(r["x"] - c["xstar"]) <= 1e-13 * np.linalg.norm(c["xstar"])
+    z = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], np.zeros(c["n"]), 2)
+    assert z["status"] == 0 and z["iters"] == 0 and np.all(z["x"] == 0)
+    # x0 != 0 path: same answer as x0 = 0
+    x0 = np.random.default_rng(5).uniform(-1, 1, c["n"])
+    a = oracle_mod.sstep(*args, 3, rtol=1e-10, x0=x0)
+    assert a["status"] == 0 and np.linalg.norm(a["x"] - c["xstar"]) <= 1e-8 * np.linalg.norm(c["xstar"])
+
+
+# (g) -------------------------------------------------------------------------
+@pytest.mark.slow
+def test_paper_514_iterations(oracle_mod):
+    """250^3 Poisson, rhs = 1, no preconditioner (== Jacobi on a
+    constant diagonal), rtol = 1e-6: PFCG and PCGs(s=1) take 514 iterations on one GPU."""
+    with open(os.path.join(GOLDEN, "paper_iterations.txt")) as f:
+        gold = {k: int(v) for k, v in (ln.split("#")[0].split() for ln in f if ln.strip() and not ln.startswith("#"))}
+    c = gen.make_config(6)
+    assert c["n"] == 250 ** 3 and c["nnz"] == 109_000_000
+    res = oracle_mod.pfcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=1e-6, maxit=2000)
+    assert res["status"] == 0 and res["iters"] == gold["pfcg_250cubed_1gpu"]
