@@ -1,0 +1,144 @@
+/*
+ * sstep_cg.h -- C ABI of the B200-native s-step preconditioned CG hot path
+ * (Chronopoulos-Gear s-step PCG as described in arxiv 2501.03743).
+ *
+ * Problem statement: solve A x = b, A symmetric positive definite, with an spd
+ * preconditioner B (Eq. 1).  Solver signature
+ * PCGs(A, b, B, x0, s, rtol, kmax) (Alg. 3); B = diag(A) here.
+ *
+ * One OUTER iteration (Alg. 3 l.5-21) is, on the device, in one CUDA graph:
+ *   a1  matrix-powers kernel, Alg. 4: R_1 = D^-1 r and, for
+ *       j = 1..s, AR_j = A R_j, R_{j+1} = D^-1 AR_j  (s Jacobi-fused CSR SpMVs)
+ *   a2  fused block inner products in one pass (Eq. 3-4, PAPER.md:142-154;
+ *       generalises Alg. 5): M = R^T AR, C = AP^T R, m = R^T r
+ *   a3  on-device s x s solves: W_prev beta = -C,
+ *       W = M + C^T beta, W alpha = m   (Cholesky, one warp)
+ *   a4  fused block updates (Alg. 3 l.17-21): P <- R + P beta, AP <- AR + AP beta,
+ *       x <- x + P alpha, r <- r - AP alpha, plus R_1 <- D^-1 r and ||r||^2
+ *   a5  stop test ||r||_2 < rtol * ||r_0||_2 (Alg. 3 l.31-33)
+ *
+ * General rules
+ *   - All functions return an int: 0 = success / converged, > 0 = solver
+ *     outcome (see SSTEP_CG_* below), < 0 = invalid argument or CUDA error
+ *     (text via sstep_cg_last_error).  No exceptions, no global state.
+ *   - Pointers are DEVICE pointers unless the name ends in _host.  fp64 values,
+ *     int32 indices.  All work is enqueued on the stream given at create();
+ *     functions that return results to the host synchronise that stream.
+ *   - CSR: 0-based, rowptr[n+1], colidx[nnz], vals[nnz]; every row holds its
+ *     diagonal entry and it is > 0.  Column order inside a row is free.
+ *     The three arrays are BORROWED: the caller keeps them alive and unchanged
+ *     until sstep_cg_destroy or the next sstep_cg_setup.
+ *   - n x s blocks in the test hooks use two layouts:
+ *       column-major ("cm"): element (i, j) at X[j*n + i]   -- R, AR
+ *       interleaved  ("il"): element (i, j) at X[i*s + j]   -- P, AP
+ *     small s x s matrices are row-major: W[i*s + j].
+ *   - There is no CPU fallback: every entry point fails with
+ *     SSTEP_CG_ERR_CUDA if no sm_100 device is usable.
+ */
+#ifndef SSTEP_CG_H
+#define SSTEP_CG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SSTEP_CG_SMAX 16           /* largest supported block size s */
+
+/* solver outcomes (return value of solve / field status) */
+#define SSTEP_CG_CONVERGED 0       /* ||r|| < rtol ||r0||                                   */
+#define SSTEP_CG_MAXIT 1           /* "did not converge within kmax iterations"; x valid */
+#define SSTEP_CG_BREAKDOWN 2       /* non-positive / non-finite Cholesky pivot or NaN; x = last good iterate */
+/* errors */
+#define SSTEP_CG_ERR_ARG (-1)
+#define SSTEP_CG_ERR_CUDA (-2)
+#define SSTEP_CG_ERR_STATE (-3)    /* call order violated (e.g. solve before setup) */
+#define SSTEP_CG_ERR_MATRIX (-4)   /* rowptr inconsistent, missing or non-positive diagonal */
+
+/* basis of the matrix-powers kernel */
+#define SSTEP_CG_BASIS_MONOMIAL 0  /* the paper's basis, Alg. 4 */
+#define SSTEP_CG_BASIS_CHEBYSHEV 1 /* Chebyshev on [0,2] for D^-1 A (NEXT-1) */
+
+typedef struct sstep_cg sstep_cg_t;
+
+typedef struct sstep_cg_result {
+    int32_t status;          /* SSTEP_CG_CONVERGED / MAXIT / BREAKDOWN */
+    int32_t outer_iters;     /* outer iterations executed */
+    int64_t cg_equiv_iters;  /* s * outer_iters ("one iteration of PCGs corresponds to s iterations") */
+    double relres;           /* ||r||_2 / ||r_0||_2, recurrence residual, at exit */
+    double r0_norm;          /* ||r_0||_2 */
+    double solve_seconds;    /* host wall time of the call (informative) */
+    int64_t kernel_launches; /* kernels this call enqueued (graph nodes x replays + init) */
+} sstep_cg_result;
+
+/* Create a solver bound to CUDA device `device` and to `cuda_stream` (a
+ * cudaStream_t passed as void*, borrowed; NULL = the legacy default stream).
+ * Allocates nothing problem-sized. */
+int sstep_cg_create(sstep_cg_t **handle, int device, void *cuda_stream);
+
+/* Bind a matrix and a block size.  Validates (n > 0, 1 <= s <= SSTEP_CG_SMAX,
+ * rowptr[0] = 0, rowptr[n] = nnz, diagonal present and > 0), computes
+ * dinv = 1/a_ii, picks the SpMV variant from the row-length statistics,
+ * allocates the workspaces (R, AR, P, AP: n x s each; x, r, dinv: n) and
+ * captures the outer iteration into a CUDA graph.  Re-callable. */
+int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *rowptr,
+                   const int32_t *colidx, const double *vals, int s);
+
+/* Options, to be set between create and setup (unknown key -> ERR_ARG):
+ *   "basis"        0 monomial (default) | 1 chebyshev
+ *   "spmv_variant" 0 auto (default) | 1 force the generic vector-per-row kernel | 2 force the bulk-staged kernel
+ *   "lanes"        0 auto | 1,2,4,8,16,32 lanes per row
+ *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
+int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
+int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);
+
+/* Solve A x = b from x0 (NULL = zeros).  `x` is caller-owned output and may
+ * alias x0.  Runs until ||r||_2 < rtol ||r_0||_2 (strict; recurrence
+ * residual), `maxit` OUTER iterations, or breakdown.  Returns the status that
+ * is also stored in out->status (out may be NULL). */
+int sstep_cg_solve(sstep_cg_t *handle, const double *b, const double *x0, double *x,
+                   double rtol, int maxit, sstep_cg_result *out);
+
+/* The same solve in three steps, for timing exactly k outer iterations:
+ *   begin   : r = b - A x0, R_1 = D^-1 r, P = AP = 0, W_prev = I, k = 0 (asynchronous)
+ *   iterate : enqueue `k_outer` replays of the outer-iteration graph (asynchronous, no
+ *             host synchronisation; iterations after convergence/breakdown exit early on a device flag)
+ *   end     : copy x out, synchronise, fill `out` */
+int sstep_cg_solve_begin(sstep_cg_t *handle, const double *b, const double *x0, double rtol);
+int sstep_cg_iterate(sstep_cg_t *handle, int k_outer);
+int sstep_cg_solve_end(sstep_cg_t *handle, double *x, sstep_cg_result *out);
+
+/* End-to-end convenience with HOST buffers: uploads CSR, b, x0 (NULL = zeros),
+ * runs setup + solve on a private device copy, downloads x.  This is the call
+ * bench.py's `e2e` number times. */
+int sstep_cg_solve_host(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *rowptr_host,
+                        const int32_t *colidx_host, const double *vals_host, const double *b_host,
+                        const double *x0_host, double *x_host, int s, double rtol, int maxit,
+                        sstep_cg_result *out);
+
+int sstep_cg_destroy(sstep_cg_t *handle);
+
+/* Text of the last failure on this handle ("" if none).  Never NULL. */
+const char *sstep_cg_last_error(sstep_cg_t *handle);
+
+/* ---- test hooks: run exactly the production kernels on caller-supplied device buffers ---- */
+
+/* a1, one SpMV of the matrix-powers kernel: y = A x; if yjac != NULL also yjac = D^-1 y. */
+int sstep_cg_test_spmv(sstep_cg_t *handle, const double *x, double *y, double *yjac);
+/* a1, Alg. 4: R(:,1) = D^-1 r, then the s fused SpMVs.  R, AR column-major n x s. */
+int sstep_cg_test_mpk(sstep_cg_t *handle, const double *r, double *R_cm, double *AR_cm);
+/* a2: M = R^T AR, C = AP^T R, m = R^T r.  R, AR column-major; AP interleaved; M, C (s*s), m (s) device outputs. */
+int sstep_cg_test_gram(sstep_cg_t *handle, const double *R_cm, const double *AR_cm, const double *AP_il,
+                       const double *r, double *M, double *C, double *m);
+/* a3: beta = -Wprev^-1 C, W = M + C^T beta, alpha = W^-1 m; status_out[0] = 0 or SSTEP_CG_BREAKDOWN. */
+int sstep_cg_test_small_solve(sstep_cg_t *handle, const double *M, const double *C, const double *m,
+                              const double *Wprev, double *beta, double *alpha, double *W, int32_t *status_out);
+/* a4, in place: P, AP (interleaved), x, r updated; R_cm(:,1) <- D^-1 r_new; rho_out[0] = ||r_new||^2. */
+int sstep_cg_test_update(sstep_cg_t *handle, double *R_cm, const double *AR_cm, double *P_il, double *AP_il,
+                         double *x, double *r, const double *beta, const double *alpha, double *rho_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SSTEP_CG_H */

@@ -1,0 +1,277 @@
+"""paper_2501_03743_b200 -- thin Python binding of the C-ABI library libsstepcg.so (include/sstep_cg.h).
+
+Argument marshalling only: every step of the hot path (Jacobi-fused CSR SpMV / matrix-powers kernel, fused
+Gram blocks, on-device s x s solves, fused block updates, graph-captured solve loop) runs in the hand-written
+sm_100a kernels under csrc/.  PyTorch is used for device memory and streams.  There is no CPU fallback: if the
+library is missing or no B200-class device is present, the calls raise.
+
+Block conventions of the Python face: an n x s block is a torch tensor of shape (s, n) whose row j is column j
+of the paper's block.  The R / AR blocks are passed to the kernels as they are ("column-major");
+P / AP are transposed to the interleaved (n, s) layout the kernels use.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from .build import LIB, build_library
+
+__all__ = ["SStepCG", "SStepCGError", "load_library", "STATUS_NAMES", "EXPORTED_SYMBOLS"]
+
+SMAX = 16
+STATUS_NAMES = {0: "converged", 1: "maxit", 2: "breakdown"}
+EXPORTED_SYMBOLS = [
+    "sstep_cg_create", "sstep_cg_setup", "sstep_cg_set_option", "sstep_cg_get_info", "sstep_cg_solve",
+    "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_solve_host", "sstep_cg_destroy",
+    "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_gram",
+    "sstep_cg_test_small_solve", "sstep_cg_test_update",
+]
+
+
+class SStepCGError(RuntimeError):
+    pass
+
+
+class _Result(C.Structure):
+    _fields_ = [("status", C.c_int32), ("outer_iters", C.c_int32), ("cg_equiv_iters", C.c_int64),
+                ("relres", C.c_double), ("r0_norm", C.c_double), ("solve_seconds", C.c_double),
+                ("kernel_launches", C.c_int64)]
+
+    def as_dict(self):
+        d = {k: getattr(self, k) for k, _ in self._fields_}
+        d["status_name"] = STATUS_NAMES.get(d["status"], str(d["status"]))
+        return d
+
+
+_lib = None
+
+
+def load_library(build: bool = True):
+    """dlopen libsstepcg.so (building it with nvcc first if it is missing or stale) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build:
+        build_library()
+    if not os.path.exists(LIB):
+        raise SStepCGError(f"{LIB} is missing: run `python -c 'import __graft_entry__ as g; g.build()'`")
+    lib = C.CDLL(LIB)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
+    lib.sstep_cg_create.argtypes = [C.POINTER(vp), i32, vp]
+    lib.sstep_cg_setup.argtypes = [vp, i64, i64, vp, vp, vp, i32]
+    lib.sstep_cg_set_option.argtypes = [vp, C.c_char_p, i64]
+    lib.sstep_cg_get_info.argtypes = [vp, C.c_char_p, C.POINTER(i64)]
+    lib.sstep_cg_solve.argtypes = [vp, vp, vp, vp, dbl, i32, C.POINTER(_Result)]
+    lib.sstep_cg_solve_begin.argtypes = [vp, vp, vp, dbl]
+    lib.sstep_cg_iterate.argtypes = [vp, i32]
+    lib.sstep_cg_solve_end.argtypes = [vp, vp, C.POINTER(_Result)]
+    lib.sstep_cg_solve_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, dbl, i32, C.POINTER(_Result)]
+    lib.sstep_cg_destroy.argtypes = [vp]
+    lib.sstep_cg_last_error.argtypes = [vp]
+    lib.sstep_cg_last_error.restype = C.c_char_p
+    lib.sstep_cg_test_spmv.argtypes = [vp, vp, vp, vp]
+    lib.sstep_cg_test_mpk.argtypes = [vp, vp, vp, vp]
+    lib.sstep_cg_test_gram.argtypes = [vp] + [vp] * 7
+    lib.sstep_cg_test_small_solve.argtypes = [vp] + [vp] * 8
+    lib.sstep_cg_test_update.argtypes = [vp] + [vp] * 9
+    for name in EXPORTED_SYMBOLS:
+        if name != "sstep_cg_last_error":
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _torch():
+    import torch
+    return torch
+
+
+class SStepCG:
+    """One solver handle (sstep_cg_create ... sstep_cg_destroy)."""
+
+    def __init__(self, device: int = 0, stream: int | None = None, **options):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise SStepCGError("no CUDA device: the s-step PCG path has no CPU fallback")
+        self._lib = load_library()
+        self.device = device
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        self._h = C.c_void_p()
+        rc = self._lib.sstep_cg_create(C.byref(self._h), device, C.c_void_p(stream))
+        if rc:
+            self._h = None
+            raise SStepCGError(f"sstep_cg_create failed ({rc}): needs an sm_100 device")
+        self._keep = []
+        self.n = self.s = None
+        for k, v in options.items():
+            self.set_option(k, v)
+
+    # ------------------------------------------------------------------ helpers
+    def _check(self, rc, what):
+        if rc < 0:
+            raise SStepCGError(f"{what} failed ({rc}): {self._lib.sstep_cg_last_error(self._h).decode()}")
+        return rc
+
+    def _dev(self, t, dtype, name, numel=None):
+        torch = _torch()
+        if t is None:
+            return None
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+            raise SStepCGError(f"{name}: need a contiguous CUDA tensor of dtype {dtype}")
+        if numel is not None and t.numel() != numel:
+            raise SStepCGError(f"{name}: expected {numel} elements, got {t.numel()}")
+        return t
+
+    @staticmethod
+    def _ptr(t):
+        return C.c_void_p(0 if t is None else t.data_ptr())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.sstep_cg_destroy(self._h)
+            self._h = None
+            self._keep = []
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # ------------------------------------------------------------------ API (same names as the C ABI)
+    def set_option(self, key: str, value: int):
+        self._check(self._lib.sstep_cg_set_option(self._h, key.encode(), int(value)), "sstep_cg_set_option")
+
+    def get_info(self, key: str) -> int:
+        v = C.c_int64(0)
+        self._check(self._lib.sstep_cg_get_info(self._h, key.encode(), C.byref(v)), "sstep_cg_get_info")
+        return v.value
+
+    def setup(self, rowptr, colidx, vals, s: int):
+        torch = _torch()
+        rowptr = self._dev(rowptr, torch.int32, "rowptr")
+        colidx = self._dev(colidx, torch.int32, "colidx")
+        vals = self._dev(vals, torch.float64, "vals", colidx.numel())
+        n, nnz = rowptr.numel() - 1, colidx.numel()
+        self._check(self._lib.sstep_cg_setup(self._h, n, nnz, self._ptr(rowptr), self._ptr(colidx), self._ptr(vals), int(s)),
+                    "sstep_cg_setup")
+        self._keep = [rowptr, colidx, vals]  # borrowed by the library until the next setup / destroy
+        self.n, self.nnz, self.s = n, nnz, int(s)
+
+    def solve(self, b, x0=None, rtol: float = 1e-8, maxit: int = 2000):
+        torch = _torch()
+        b = self._dev(b, torch.float64, "b", self.n)
+        x0 = self._dev(x0, torch.float64, "x0", self.n)
+        x = torch.empty_like(b)
+        res = _Result()
+        self._check(self._lib.sstep_cg_solve(self._h, self._ptr(b), self._ptr(x0), self._ptr(x), float(rtol), int(maxit),
+                                             C.byref(res)), "sstep_cg_solve")
+        return x, res.as_dict()
+
+    def solve_begin(self, b, x0=None, rtol: float = 0.0):
+        torch = _torch()
+        b = self._dev(b, torch.float64, "b", self.n)
+        x0 = self._dev(x0, torch.float64, "x0", self.n)
+        self._check(self._lib.sstep_cg_solve_begin(self._h, self._ptr(b), self._ptr(x0), float(rtol)), "sstep_cg_solve_begin")
+        self._solve_keep = [b, x0]
+
+    def iterate(self, k_outer: int):
+        self._check(self._lib.sstep_cg_iterate(self._h, int(k_outer)), "sstep_cg_iterate")
+
+    def solve_end(self, want_x: bool = True):
+        torch = _torch()
+        x = torch.empty(self.n, dtype=torch.float64, device=f"cuda:{self.device}") if want_x else None
+        res = _Result()
+        self._check(self._lib.sstep_cg_solve_end(self._h, self._ptr(x), C.byref(res)), "sstep_cg_solve_end")
+        return x, res.as_dict()
+
+    def solve_host(self, rowptr, colidx, vals, b, s: int, x0=None, rtol: float = 1e-8, maxit: int = 2000, x_out=None):
+        """End-to-end call with HOST buffers (CPU torch tensors, ideally pinned)."""
+        torch = _torch()
+
+        def host(t, dtype, name):
+            if t is None:
+                return None
+            if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+                raise SStepCGError(f"{name}: need a contiguous CPU tensor of dtype {dtype}")
+            return t
+        rowptr, colidx = host(rowptr, torch.int32, "rowptr"), host(colidx, torch.int32, "colidx")
+        vals, b, x0 = host(vals, torch.float64, "vals"), host(b, torch.float64, "b"), host(x0, torch.float64, "x0")
+        n, nnz = rowptr.numel() - 1, colidx.numel()
+        x = x_out if x_out is not None else torch.empty(n, dtype=torch.float64)
+        res = _Result()
+        self._check(self._lib.sstep_cg_solve_host(self._h, n, nnz, self._ptr(rowptr), self._ptr(colidx), self._ptr(vals),
+                                                  self._ptr(b), self._ptr(x0), self._ptr(x), int(s), float(rtol), int(maxit),
+                                                  C.byref(res)), "sstep_cg_solve_host")
+        self.n, self.nnz, self.s = n, nnz, int(s)
+        return x, res.as_dict()
+
+    # ------------------------------------------------------------------ test hooks
+    def test_spmv(self, x, jacobi: bool = True):
+        torch = _torch()
+        x = self._dev(x, torch.float64, "x", self.n)
+        y = torch.empty_like(x)
+        yjac = torch.empty_like(x) if jacobi else None
+        self._check(self._lib.sstep_cg_test_spmv(self._h, self._ptr(x), self._ptr(y), self._ptr(yjac)), "sstep_cg_test_spmv")
+        return y, yjac
+
+    def test_mpk(self, r):
+        torch = _torch()
+        r = self._dev(r, torch.float64, "r", self.n)
+        R = torch.empty((self.s, self.n), dtype=torch.float64, device=r.device)
+        AR = torch.empty_like(R)
+        self._check(self._lib.sstep_cg_test_mpk(self._h, self._ptr(r), self._ptr(R), self._ptr(AR)), "sstep_cg_test_mpk")
+        return R, AR
+
+    def test_gram(self, R, AR, AP, r):
+        torch = _torch()
+        ns = self.n * self.s
+        R, AR = self._dev(R, torch.float64, "R", ns), self._dev(AR, torch.float64, "AR", ns)
+        AP_il = self._dev(AP, torch.float64, "AP", ns).t().contiguous()      # (s, n) -> interleaved (n, s)
+        r = self._dev(r, torch.float64, "r", self.n)
+        s = self.s
+        M = torch.empty((s, s), dtype=torch.float64, device=r.device)
+        Cm = torch.empty_like(M)
+        m = torch.empty(s, dtype=torch.float64, device=r.device)
+        self._check(self._lib.sstep_cg_test_gram(self._h, self._ptr(R), self._ptr(AR), self._ptr(AP_il), self._ptr(r),
+                                                 self._ptr(M), self._ptr(Cm), self._ptr(m)), "sstep_cg_test_gram")
+        return M, Cm, m
+
+    def test_small_solve(self, M, Cm, m, Wprev):
+        torch = _torch()
+        s = self.s
+        M, Cm, Wprev = (self._dev(t, torch.float64, nm, s * s) for t, nm in ((M, "M"), (Cm, "C"), (Wprev, "Wprev")))
+        m = self._dev(m, torch.float64, "m", s)
+        beta = torch.zeros((s, s), dtype=torch.float64, device=M.device)
+        alpha = torch.zeros(s, dtype=torch.float64, device=M.device)
+        W = torch.zeros_like(beta)
+        st = torch.zeros(1, dtype=torch.int32, device=M.device)
+        self._check(self._lib.sstep_cg_test_small_solve(self._h, self._ptr(M), self._ptr(Cm), self._ptr(m), self._ptr(Wprev),
+                                                        self._ptr(beta), self._ptr(alpha), self._ptr(W), self._ptr(st)),
+                    "sstep_cg_test_small_solve")
+        return int(st.item()), beta, alpha, W
+
+    def test_update(self, R, AR, P, AP, x, r, beta, alpha):
+        """Returns new (P, AP, x, r) as (s, n)/(n,) tensors plus R1 = D^-1 r_new and rho = ||r_new||^2; inputs are not modified."""
+        torch = _torch()
+        ns, s = self.n * self.s, self.s
+        R = self._dev(R, torch.float64, "R", ns).clone()
+        AR = self._dev(AR, torch.float64, "AR", ns)
+        P_il = self._dev(P, torch.float64, "P", ns).t().contiguous()
+        AP_il = self._dev(AP, torch.float64, "AP", ns).t().contiguous()
+        x = self._dev(x, torch.float64, "x", self.n).clone()
+        r = self._dev(r, torch.float64, "r", self.n).clone()
+        beta = self._dev(beta, torch.float64, "beta", s * s)
+        alpha = self._dev(alpha, torch.float64, "alpha", s)
+        rho = torch.zeros(1, dtype=torch.float64, device=x.device)
+        self._check(self._lib.sstep_cg_test_update(self._h, self._ptr(R), self._ptr(AR), self._ptr(P_il), self._ptr(AP_il),
+                                                   self._ptr(x), self._ptr(r), self._ptr(beta), self._ptr(alpha), self._ptr(rho)),
+                    "sstep_cg_test_update")
+        return P_il.t().contiguous(), AP_il.t().contiguous(), x, r, R[0].clone(), float(rho.item())

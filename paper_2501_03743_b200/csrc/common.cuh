@@ -1,0 +1,100 @@
+// common.cuh -- device helpers shared by the sm_100a kernels of the s-step PCG hot path.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define SCG_SMAX 16
+#define SCG_WARP 32
+
+// Device-resident solver state: everything the outer iteration needs that is not problem-sized.
+// Written by the kernels, read by the host only through an async copy of the header.
+struct ScgState {
+    // ---- header (copied to the host when polling) ----
+    int32_t status;      // -1 running, 0 converged, 2 breakdown
+    int32_t k;           // outer iterations completed
+    double rho;          // ||r||^2 after the last completed iteration
+    double rho0;         // ||r_0||^2
+    double rtol;         // stop when sqrt(rho) < rtol * sqrt(rho0)  (Alg. 3 l.31)
+    // ---- small dense state ----
+    double W[SCG_SMAX * SCG_SMAX];      // W of the previous outer iteration (P^T A P), row-major
+    double beta[SCG_SMAX * SCG_SMAX];
+    double alpha[SCG_SMAX];
+    double M[SCG_SMAX * SCG_SMAX];
+    double C[SCG_SMAX * SCG_SMAX];
+    double m[SCG_SMAX];
+    // ---- cross-block finish tickets (reset by the last block, so graphs can be replayed) ----
+    unsigned int ticket_gram;
+    unsigned int ticket_update;
+    unsigned int ticket_init;
+};
+#define SCG_RUNNING (-1)
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <int L>
+__device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+    for (int o = L / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ---- mbarrier + 1-D bulk async copy (TMA engine, cp.async.bulk) -------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// global -> shared bulk copy; dst/src 16 B aligned, bytes a multiple of 16; completes on `bar` (complete_tx).
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar,
+                                         uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// streaming (read-once) 128-bit and 64-bit global loads
+__device__ __forceinline__ double2 ldg_stream2(const double* p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ldg_stream(const double* p) {
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}

@@ -1,0 +1,190 @@
+// spmv.cuh -- step a1 of the hot path: one Jacobi-fused CSR SpMV of the matrix-powers kernel
+// (Alg. 4):  y = A x  (AR_j = A R_j)  and, in the epilogue,
+//   mode 0 (monomial):        yjac = dinv .* y                      (R_{j+1} = B^-1 AR_j)
+//   mode 1 (Chebyshev, j=1):  yjac = dinv .* y - x                  (R_2 = Z R_1,  Z = D^-1 A - I)
+//   mode 2 (Chebyshev, j>1):  yjac = 2 (dinv .* y - x) - xprev      (R_{j+1} = 2 Z R_j - R_{j-1})
+// Two variants, chosen at setup from the row-length statistics:
+//   spmv_vec_kernel  : generic vector-per-row (L lanes per row, L in {1..32}); any CSR.
+//   spmv_bulk_kernel : per-warp multi-stage pipeline; the warp's slice of colidx/vals is streamed into
+//                      shared memory by the TMA engine (cp.async.bulk, 16 B aligned, L2 evict-first) while the
+//                      warp gathers x for the previous tile.  Needs every tile of 32/L rows to hold < CAP-3 nnz.
+#pragma once
+#include "common.cuh"
+
+__device__ __forceinline__ void spmv_epilogue(int64_t row, double acc, const double* __restrict__ dinv,
+                                              const double* __restrict__ x, const double* __restrict__ xprev, int mode,
+                                              double* __restrict__ y, double* __restrict__ yjac) {
+    y[row] = acc;
+    if (yjac) {
+        double z = dinv[row] * acc;
+        if (mode == 1) z = z - x[row];
+        else if (mode == 2) z = 2.0 * (z - x[row]) - xprev[row];
+        yjac[row] = z;
+    }
+}
+
+template <int L>
+__global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci,
+                                                       const double* __restrict__ va, const double* __restrict__ dinv,
+                                                       const double* __restrict__ x, double* __restrict__ y,
+                                                       double* __restrict__ yjac, const double* __restrict__ xprev, int mode,
+                                                       const ScgState* __restrict__ st) {
+    if (st && st->status != SCG_RUNNING) return;
+    const int g = threadIdx.x % L;
+    const int64_t rows_per_pass = (int64_t)gridDim.x * (blockDim.x / L);
+    // the loop runs on the warp's first row so that all 32 lanes reach the shuffles the same number of times
+    const int warp_rows = 32 / L;
+    for (int64_t wrow = (int64_t)blockIdx.x * (blockDim.x / L) + (threadIdx.x >> 5) * warp_rows; wrow < n;
+         wrow += rows_per_pass) {
+        const int64_t row = wrow + (threadIdx.x & 31) / L;
+        const bool live = row < n;
+        int lo = 0, hi = 0;
+        if (live) { lo = rp[row]; hi = rp[row + 1]; }
+        double acc = 0.0;
+        for (int k = lo + g; k < hi; k += L) acc = fma(va[k], x[ci[k]], acc);
+        acc = group_sum<L>(acc);
+        if (live && g == 0) spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Bulk-staged variant.  One warp owns a ring of D slots; slot = { double vals[CAP]; int cols[CAP] }.
+// Tile t covers rows [t*RPT, (t+1)*RPT), RPT = 32/L; its nnz range [rp[row0], rp[row1]) is copied from the
+// 16 B aligned element a0 = rp[row0] & ~3 on.  Tiles are dealt to warps round-robin so that at any time the
+// grid works on one contiguous window of rows (keeps the gathered vector's working set in L2/L1).
+template <int L, int D, int CAP, int WPC>
+__global__ void __launch_bounds__(WPC * 32) spmv_bulk_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp,
+                                                             const int* __restrict__ ci, const double* __restrict__ va,
+                                                             const double* __restrict__ dinv, const double* __restrict__ x,
+                                                             double* __restrict__ y, double* __restrict__ yjac,
+                                                             const double* __restrict__ xprev, int mode,
+                                                             const ScgState* __restrict__ st, int64_t num_tiles) {
+    if (st && st->status != SCG_RUNNING) return;
+    constexpr int RPT = 32 / L;
+    constexpr int U = (L == 1) ? 8 : 4;  // predicated unroll of the gather loop
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* svals = reinterpret_cast<double*>(smem_raw) + (size_t)warp * D * CAP;
+    int* scols = reinterpret_cast<int*>(smem_raw + (size_t)WPC * D * CAP * sizeof(double)) + (size_t)warp * D * CAP;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)WPC * D * CAP * 12) + warp * D;
+
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < D; d++) mbar_init(&bars[d], 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    const uint64_t policy = l2_policy_evict_first();
+    const int64_t GW = (int64_t)gridDim.x * WPC;
+    const int64_t gw = (int64_t)blockIdx.x * WPC + warp;
+    if (gw >= num_tiles) return;
+    const int64_t my_tiles = (num_tiles - gw + GW - 1) / GW;
+
+    // issue the copies of this warp's i-th tile into slot i % D; nz0/nz1 = its nnz range (valid in lane 0)
+    auto issue = [&](int64_t i, int nz0, int nz1) {
+        const int sl = (int)(i % D);
+        const int a0 = nz0 & ~3;
+        int bulk_end = (nz1 + 3) & ~3;
+        const int lim = (int)(nnz & ~(int64_t)3);
+        if (bulk_end > lim) bulk_end = lim;
+        if (bulk_end < a0) bulk_end = a0;
+        const int cnt = bulk_end - a0;
+        double* dv = svals + sl * CAP;
+        int* dc = scols + sl * CAP;
+        if (lane == 0) {
+            fence_proxy_async_smem();
+            if (cnt > 0) {
+                mbar_expect_tx(&bars[sl], (uint32_t)cnt * 12u);
+                bulk_g2s(dv, va + a0, (uint32_t)cnt * 8u, &bars[sl], policy);
+                bulk_g2s(dc, ci + a0, (uint32_t)cnt * 4u, &bars[sl], policy);
+            } else {
+                mbar_arrive(&bars[sl]);
+            }
+        }
+        // ragged tail of the arrays (at most 3 elements of the whole matrix) by plain loads
+        const int b_end = __shfl_sync(0xffffffffu, bulk_end, 0);
+        const int b_a0 = __shfl_sync(0xffffffffu, a0, 0);
+        const int b_nz1 = __shfl_sync(0xffffffffu, nz1, 0);
+        for (int e = b_end + lane; e < b_nz1; e += 32) {
+            dv[e - b_a0] = va[e];
+            dc[e - b_a0] = ci[e];
+        }
+    };
+    auto tile_bounds = [&](int64_t i, int& nz0, int& nz1) {  // lane 0 only
+        const int64_t t = gw + i * GW;
+        const int64_t row0 = t * RPT;
+        int64_t row1 = row0 + RPT;
+        if (row1 > n) row1 = n;
+        nz0 = rp[row0];
+        nz1 = rp[row1];
+    };
+
+    // prologue: fill D-1 slots
+    int nb0 = 0, nb1 = 0;  // bounds of the next tile to issue (prefetched one iteration ahead)
+    for (int64_t i = 0; i < D - 1 && i < my_tiles; i++) {
+        int a = 0, b = 0;
+        if (lane == 0) tile_bounds(i, a, b);
+        issue(i, a, b);
+    }
+    if (lane == 0 && D - 1 < my_tiles) tile_bounds(D - 1, nb0, nb1);
+    // per-row bounds of the first tile
+    const int g = lane % L;
+    int lo_n = 0, hi_n = 0;
+    {
+        const int64_t row = gw * RPT + lane / L;
+        if (row < n) { lo_n = rp[row]; hi_n = rp[row + 1]; }
+    }
+    for (int64_t i = 0; i < my_tiles; i++) {
+        const int64_t t = gw + i * GW;
+        const int64_t row = t * RPT + lane / L;
+        const int lo = lo_n, hi = hi_n;
+        // prefetch: per-row bounds of tile i+1, nnz range of tile i+D; issue tile i+D-1 into the slot freed last
+        if (i + 1 < my_tiles) {
+            const int64_t rown = row + GW * RPT;
+            lo_n = hi_n = 0;
+            if (rown < n) { lo_n = rp[rown]; hi_n = rp[rown + 1]; }
+        }
+        if (i + D - 1 < my_tiles) {
+            issue(i + D - 1, nb0, nb1);
+            if (lane == 0 && i + D < my_tiles) tile_bounds(i + D, nb0, nb1);
+        }
+        const int sl = (int)(i % D);
+        const int a0 = __shfl_sync(0xffffffffu, lo, 0) & ~3;
+        mbar_wait(&bars[sl], (uint32_t)((i / D) & 1));
+        const double* sv = svals + sl * CAP - a0;
+        const int* sc = scols + sl * CAP - a0;
+        double acc = 0.0;
+        for (int k = lo + g; k < hi; k += U * L) {
+            int c[U];
+            double v[U], xv[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int kk = k + u * L;
+                const bool ok = kk < hi;
+                c[u] = ok ? sc[kk] : -1;
+                v[u] = ok ? sv[kk] : 0.0;
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
+#pragma unroll
+            for (int u = 0; u < U; u++) acc = fma(v[u], xv[u], acc);
+        }
+        acc = group_sum<L>(acc);
+        if (g == 0 && row < n) spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
+        __syncwarp();
+    }
+}
+
+// max nnz over tiles of `rpt` rows (setup-time check for the bulk variant)
+__global__ void tile_nnz_max_kernel(int64_t n, const int* __restrict__ rp, int rpt, int64_t num_tiles, int* __restrict__ out) {
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int m = 0;
+    if (t < num_tiles) {
+        int64_t r0 = t * rpt, r1 = r0 + rpt;
+        if (r1 > n) r1 = n;
+        m = rp[r1] - rp[r0];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}

@@ -1,0 +1,646 @@
+// sstep_cg.cu -- C ABI (include/sstep_cg.h) of the B200-native s-step PCG hot path: handle, setup,
+// CUDA-graph capture of one outer iteration, the solve loop, and the test hooks.  sm_100a only, no CPU fallback.
+#include "sstep_cg.h"
+
+#include <chrono>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "common.cuh"
+#include "gram.cuh"
+#include "spmv.cuh"
+#include "update.cuh"
+
+namespace {
+
+struct Header {  // mirrors the first fields of ScgState
+    int32_t status, k;
+    double rho, rho0, rtol;
+};
+
+constexpr int BULK_D = 3, BULK_CAP = 256, BULK_WPC = 8;
+constexpr size_t BULK_SMEM = (size_t)BULK_WPC * BULK_D * BULK_CAP * 12 + (size_t)BULK_WPC * BULK_D * 8;
+
+}  // namespace
+
+struct sstep_cg {
+    int device = 0;
+    cudaStream_t stream = nullptr;      // borrowed
+    cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
+    int num_sms = 0;
+    // options
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1;
+    // problem (borrowed CSR)
+    int64_t n = 0, nnz = 0;
+    int s = 0;
+    const int* rp = nullptr;
+    const int* ci = nullptr;
+    const double* va = nullptr;
+    bool ready = false, in_solve = false;
+    // owned device memory
+    double *dinv = nullptr, *R = nullptr, *AR = nullptr, *P = nullptr, *AP = nullptr, *x = nullptr, *r = nullptr;
+    double* partials = nullptr;
+    ScgState* st = nullptr;       // production state
+    ScgState* st_test = nullptr;  // state used by the test hooks
+    int* iscratch = nullptr;      // [err, max_len, max_tile]
+    // owned copies made by solve_host
+    int *own_rp = nullptr, *own_ci = nullptr;
+    double *own_va = nullptr, *own_b = nullptr, *own_x = nullptr;
+    // kernel configuration
+    int lanes = 1;
+    bool bulk = false;
+    int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0;
+    int64_t num_tiles = 0;
+    int max_row_len = 0;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    // host polling
+    Header* h_hdr = nullptr;  // pinned, 2 entries
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    // bookkeeping
+    int64_t launches = 0;
+    int64_t graph_launches = 0;
+    double rtol = 0.0;
+    std::chrono::steady_clock::time_point t_begin;
+    std::string err;
+};
+
+namespace {
+
+int fail(sstep_cg* h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+
+#define CK(call)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess)                                                                                \
+            return fail(h, SSTEP_CG_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));            \
+    } while (0)
+
+// ---------------------------------------------------------------- kernel dispatch
+template <int L>
+cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
+                          int mode, const ScgState* st) {
+    if (h->bulk) {
+        spmv_bulk_kernel<L, BULK_D, BULK_CAP, BULK_WPC><<<h->spmv_grid, BULK_WPC * 32, BULK_SMEM, sm>>>(
+            h->n, h->nnz, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, h->num_tiles);
+    } else {
+        spmv_vec_kernel<L><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spmv(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
+                        int mode, const ScgState* st) {
+    h->launches++;
+    switch (h->lanes) {
+        case 1: return launch_spmv_L<1>(h, sm, x, y, yjac, xprev, mode, st);
+        case 2: return launch_spmv_L<2>(h, sm, x, y, yjac, xprev, mode, st);
+        case 4: return launch_spmv_L<4>(h, sm, x, y, yjac, xprev, mode, st);
+        case 8: return launch_spmv_L<8>(h, sm, x, y, yjac, xprev, mode, st);
+        case 16: return launch_spmv_L<16>(h, sm, x, y, yjac, xprev, mode, st);
+        default: return launch_spmv_L<32>(h, sm, x, y, yjac, xprev, mode, st);
+    }
+}
+
+template <int L>
+cudaError_t config_spmv_L(sstep_cg* h) {
+    int occ = 0;
+    cudaError_t e;
+    if (h->bulk) {
+        auto k = spmv_bulk_kernel<L, BULK_D, BULK_CAP, BULK_WPC>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BULK_SMEM);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, BULK_WPC * 32, BULK_SMEM);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        int64_t want = (h->num_tiles + BULK_WPC - 1) / BULK_WPC;
+        int64_t cap = (int64_t)occ * h->num_sms;
+        h->spmv_grid = (int)(want < cap ? want : cap);
+    } else {
+        auto k = spmv_vec_kernel<L>;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, 0);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        int64_t rows_per_block = 256 / L;
+        int64_t want = (h->n + rows_per_block - 1) / rows_per_block;
+        int64_t cap = (int64_t)occ * h->num_sms * 4;
+        h->spmv_grid = (int)(want < cap ? want : cap);
+    }
+    if (h->spmv_grid < 1) h->spmv_grid = 1;
+    return cudaSuccess;
+}
+
+cudaError_t config_spmv(sstep_cg* h) {
+    switch (h->lanes) {
+        case 1: return config_spmv_L<1>(h);
+        case 2: return config_spmv_L<2>(h);
+        case 4: return config_spmv_L<4>(h);
+        case 8: return config_spmv_L<8>(h);
+        case 16: return config_spmv_L<16>(h);
+        default: return config_spmv_L<32>(h);
+    }
+}
+
+template <int S>
+cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R, const double* AR, const double* AP,
+                   const double* r, ScgState* st, int do_solve) {
+    using Cfg = GramCfg<S>;
+    if (configure) {
+        int occ = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_kernel<S>, Cfg::NW * 32, 0);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        int64_t want = (h->n + Cfg::RG * 32 - 1) / (Cfg::RG * 32);
+        int64_t cap = (int64_t)occ * h->num_sms;
+        h->gram_grid = (int)(want < cap ? want : cap);
+        return cudaSuccess;
+    }
+    gram_kernel<S><<<h->gram_grid, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve);
+    return cudaGetLastError();
+}
+
+template <int S>
+cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
+                     double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
+    if (configure) {
+        int occ = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_kernel<S>, 256, 0);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        int64_t want = (h->n + 255) / 256;
+        int64_t cap = (int64_t)occ * h->num_sms;
+        h->update_grid = (int)(want < cap ? want : cap);
+        return cudaSuccess;
+    }
+    update_kernel<S><<<h->update_grid, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
+    return cudaGetLastError();
+}
+
+#define SCG_DISPATCH_S(fn, ...)                          \
+    switch (h->s) {                                      \
+        case 1: return fn<1>(__VA_ARGS__);               \
+        case 2: return fn<2>(__VA_ARGS__);               \
+        case 3: return fn<3>(__VA_ARGS__);               \
+        case 4: return fn<4>(__VA_ARGS__);               \
+        case 5: return fn<5>(__VA_ARGS__);               \
+        case 6: return fn<6>(__VA_ARGS__);               \
+        case 7: return fn<7>(__VA_ARGS__);               \
+        case 8: return fn<8>(__VA_ARGS__);               \
+        case 9: return fn<9>(__VA_ARGS__);               \
+        case 10: return fn<10>(__VA_ARGS__);             \
+        case 11: return fn<11>(__VA_ARGS__);             \
+        case 12: return fn<12>(__VA_ARGS__);             \
+        case 13: return fn<13>(__VA_ARGS__);             \
+        case 14: return fn<14>(__VA_ARGS__);             \
+        case 15: return fn<15>(__VA_ARGS__);             \
+        default: return fn<16>(__VA_ARGS__);             \
+    }
+
+cudaError_t launch_gram(sstep_cg* h, cudaStream_t sm, bool configure, const double* R, const double* AR, const double* AP,
+                        const double* r, ScgState* st, int do_solve) {
+    if (!configure) h->launches++;
+    SCG_DISPATCH_S(gram_S, h, sm, configure, R, AR, AP, r, st, do_solve)
+}
+
+cudaError_t launch_update(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
+                          double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
+    if (!configure) h->launches++;
+    SCG_DISPATCH_S(update_S, h, sm, configure, R, AR, P, AP, x, r, beta, alpha, st, rho_out)
+}
+
+// Alg. 4 on the given buffers: s Jacobi-fused SpMVs (R(:,1) must already hold D^-1 r)
+cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, const ScgState* st) {
+    const int64_t n = h->n;
+    for (int j = 0; j < h->s; j++) {
+        double* yjac = (j + 1 < h->s) ? R + (int64_t)(j + 1) * n : nullptr;
+        int mode = 0;
+        const double* xprev = nullptr;
+        if (h->basis == SSTEP_CG_BASIS_CHEBYSHEV) {
+            mode = (j == 0) ? 1 : 2;
+            if (j > 0) xprev = R + (int64_t)(j - 1) * n;
+        }
+        cudaError_t e = launch_spmv(h, sm, R + (int64_t)j * n, AR + (int64_t)j * n, yjac, xprev, mode, st);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+// one outer iteration on the production buffers (Alg. 3 l.5-21)
+cudaError_t launch_outer(sstep_cg* h, cudaStream_t sm) {
+    cudaError_t e = launch_mpk(h, sm, h->R, h->AR, h->st);
+    if (e != cudaSuccess) return e;
+    e = launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1);
+    if (e != cudaSuccess) return e;
+    return launch_update(h, sm, false, h->R, h->AR, h->P, h->AP, h->x, h->r, h->st->beta, h->st->alpha, h->st, nullptr);
+}
+
+void free_problem(sstep_cg* h) {
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    h->gexec = nullptr;
+    h->graph = nullptr;
+    double** bufs[] = {&h->dinv, &h->R, &h->AR, &h->P, &h->AP, &h->x, &h->r, &h->partials};
+    for (double** b : bufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    h->ready = false;
+    h->in_solve = false;
+}
+
+void free_owned(sstep_cg* h) {
+    if (h->own_rp) cudaFree(h->own_rp);
+    if (h->own_ci) cudaFree(h->own_ci);
+    if (h->own_va) cudaFree(h->own_va);
+    if (h->own_b) cudaFree(h->own_b);
+    if (h->own_x) cudaFree(h->own_x);
+    h->own_rp = h->own_ci = nullptr;
+    h->own_va = h->own_b = h->own_x = nullptr;
+}
+
+int kernels_per_outer(const sstep_cg* h) { return h->s + 2; }
+
+}  // namespace
+
+// =============================================================================================== C ABI
+extern "C" {
+
+int sstep_cg_create(sstep_cg_t** handle, int device, void* cuda_stream) {
+    if (!handle) return SSTEP_CG_ERR_ARG;
+    *handle = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return SSTEP_CG_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SSTEP_CG_ERR_CUDA;
+    if (prop.major < 10) return SSTEP_CG_ERR_CUDA;  // sm_100a code only: fail loudly elsewhere
+    if (cudaSetDevice(device) != cudaSuccess) return SSTEP_CG_ERR_CUDA;
+    sstep_cg* h = new sstep_cg();
+    h->device = device;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->num_sms = prop.multiProcessorCount;
+    bool ok = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->st, sizeof(ScgState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->st_test, sizeof(ScgState)) == cudaSuccess;
+    ok = ok && cudaMalloc(&h->iscratch, 4 * sizeof(int)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&h->h_hdr, 2 * sizeof(Header)) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&h->ev[0], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&h->ev[1], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaMemset(h->st, 0, sizeof(ScgState)) == cudaSuccess;
+    ok = ok && cudaMemset(h->st_test, 0, sizeof(ScgState)) == cudaSuccess;
+    if (!ok) {
+        sstep_cg_destroy(h);
+        return SSTEP_CG_ERR_CUDA;
+    }
+    *handle = h;
+    return 0;
+}
+
+int sstep_cg_destroy(sstep_cg_t* h) {
+    if (!h) return SSTEP_CG_ERR_ARG;
+    cudaSetDevice(h->device);
+    cudaStreamSynchronize(h->stream);
+    free_problem(h);
+    free_owned(h);
+    if (h->st) cudaFree(h->st);
+    if (h->st_test) cudaFree(h->st_test);
+    if (h->iscratch) cudaFree(h->iscratch);
+    if (h->h_hdr) cudaFreeHost(h->h_hdr);
+    for (auto& e : h->ev)
+        if (e) cudaEventDestroy(e);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    delete h;
+    return 0;
+}
+
+const char* sstep_cg_last_error(sstep_cg_t* h) { return h ? h->err.c_str() : "null handle"; }
+
+int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
+    if (!h || !key) return SSTEP_CG_ERR_ARG;
+    const std::string k(key);
+    if (k == "basis" && (value == 0 || value == 1)) h->basis = (int)value;
+    else if (k == "spmv_variant" && value >= 0 && value <= 2) h->spmv_variant = (int)value;
+    else if (k == "lanes" && (value == 0 || value == 1 || value == 2 || value == 4 || value == 8 || value == 16 || value == 32))
+        h->lanes_opt = (int)value;
+    else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
+    else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
+    return 0;
+}
+
+int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
+    if (!h || !key || !value) return SSTEP_CG_ERR_ARG;
+    const std::string k(key);
+    if (k == "lanes") *value = h->lanes;
+    else if (k == "spmv_bulk") *value = h->bulk ? 1 : 0;
+    else if (k == "spmv_grid") *value = h->spmv_grid;
+    else if (k == "gram_grid") *value = h->gram_grid;
+    else if (k == "update_grid") *value = h->update_grid;
+    else if (k == "max_row_len") *value = h->max_row_len;
+    else if (k == "num_sms") *value = h->num_sms;
+    else if (k == "kernels_per_outer") *value = kernels_per_outer(h);
+    else if (k == "basis") *value = h->basis;
+    else if (k == "launches") *value = h->launches;
+    else return fail(h, SSTEP_CG_ERR_ARG, "unknown info key: " + k);
+    return 0;
+}
+
+int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr, const int32_t* colidx, const double* vals,
+                   int s) {
+    if (!h) return SSTEP_CG_ERR_ARG;
+    if (n <= 0 || nnz <= 0 || nnz >= (int64_t(1) << 31) || n >= (int64_t(1) << 31) || !rowptr || !colidx || !vals || s < 1 ||
+        s > SSTEP_CG_SMAX)
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: need n > 0, 0 < nnz < 2^31, non-null CSR arrays, 1 <= s <= 16");
+    CK(cudaSetDevice(h->device));
+    CK(cudaStreamSynchronize(h->stream));
+    free_problem(h);
+    h->n = n; h->nnz = nnz; h->s = s;
+    h->rp = rowptr; h->ci = colidx; h->va = vals;
+    cudaStream_t sm = h->stream;
+
+    // dinv, validation, row statistics
+    CK(cudaMalloc(&h->dinv, sizeof(double) * n));
+    CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
+    analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
+    CK(cudaGetLastError());
+    int hs[4] = {0, 0, 0, 0};
+    CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
+    CK(cudaStreamSynchronize(sm));
+    if (hs[0]) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "setup: invalid matrix (flags %d: 1 rowptr, 2 column index, 4 diagonal missing or <= 0)", hs[0]);
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_MATRIX, buf);
+    }
+    h->max_row_len = hs[1];
+
+    // SpMV variant: lanes per row from the mean row length (vector-per-row ... warp-per-row), bulk staging if every tile fits
+    const double mean = (double)nnz / (double)n;
+    int L = 1;
+    while (L < 32 && mean / L > 8.0) L *= 2;
+    if (h->lanes_opt) L = h->lanes_opt;
+    h->bulk = false;
+    const bool aligned = (((uintptr_t)colidx | (uintptr_t)vals) & 15) == 0;
+    if (h->spmv_variant != 1 && aligned) {
+        for (int Lb = L; Lb <= 32; Lb *= 2) {
+            const int rpt = 32 / Lb;
+            const int64_t tiles = (n + rpt - 1) / rpt;
+            CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
+            tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, rpt, tiles, h->iscratch + 2);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+            if (hs[2] + 3 <= BULK_CAP) {
+                h->bulk = true;
+                L = Lb;
+                h->num_tiles = tiles;
+                break;
+            }
+            if (h->lanes_opt) break;
+        }
+    }
+    if (h->spmv_variant == 2 && !h->bulk) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: bulk SpMV forced but a tile exceeds the staging capacity or arrays are not 16 B aligned");
+    }
+    h->lanes = L;
+    CK(config_spmv(h));
+    CK(launch_gram(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, 0));
+    CK(launch_update(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr));
+    {
+        int64_t want = (n + 255) / 256, cap = (int64_t)h->num_sms * 8;
+        h->init_grid = (int)(want < cap ? want : cap);
+    }
+
+    // workspaces
+    const size_t blk = sizeof(double) * (size_t)n * s;
+    CK(cudaMalloc(&h->R, blk));
+    CK(cudaMalloc(&h->AR, blk));
+    CK(cudaMalloc(&h->P, blk));
+    CK(cudaMalloc(&h->AP, blk));
+    CK(cudaMalloc(&h->x, sizeof(double) * n));
+    CK(cudaMalloc(&h->r, sizeof(double) * n));
+    size_t np = (size_t)h->gram_grid * (2 * s * s + s);
+    if (np < (size_t)h->update_grid) np = h->update_grid;
+    if (np < (size_t)h->init_grid) np = h->init_grid;
+    CK(cudaMalloc(&h->partials, sizeof(double) * np));
+    CK(cudaMemsetAsync(h->R, 0, blk, sm));
+    CK(cudaMemsetAsync(h->AR, 0, blk, sm));
+    CK(cudaMemsetAsync(h->P, 0, blk, sm));
+    CK(cudaMemsetAsync(h->AP, 0, blk, sm));
+    CK(cudaMemsetAsync(h->st, 0, sizeof(ScgState), sm));
+    CK(cudaMemsetAsync(h->st_test, 0, sizeof(ScgState), sm));
+    CK(cudaStreamSynchronize(sm));
+
+    // capture one outer iteration (s SpMVs, Gram + solves, update) into a graph
+    if (h->use_graph) {
+        const int64_t saved = h->launches;
+        CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+        cudaError_t e = launch_outer(h, h->cap_stream);
+        cudaError_t e2 = cudaStreamEndCapture(h->cap_stream, &h->graph);
+        h->launches = saved;
+        if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        CK(e2);
+        CK(cudaGraphInstantiate(&h->gexec, h->graph, 0));
+    }
+    h->ready = true;
+    return 0;
+}
+
+int sstep_cg_solve_begin(sstep_cg_t* h, const double* b, const double* x0, double rtol) {
+    if (!h || !b) return SSTEP_CG_ERR_ARG;
+    if (!h->ready) return fail(h, SSTEP_CG_ERR_STATE, "solve: call setup first");
+    if (!(rtol >= 0.0)) return fail(h, SSTEP_CG_ERR_ARG, "solve: rtol must be >= 0");
+    CK(cudaSetDevice(h->device));
+    cudaStream_t sm = h->stream;
+    h->t_begin = std::chrono::steady_clock::now();
+    h->launches = 0;
+    h->graph_launches = 0;
+    h->rtol = rtol;
+    const size_t blk = sizeof(double) * (size_t)h->n * h->s;
+    CK(cudaMemsetAsync(h->P, 0, blk, sm));
+    CK(cudaMemsetAsync(h->AP, 0, blk, sm));
+    if (x0) {  // r <- A x0 with the production SpMV, then r <- b - r in init_kernel
+        CK(launch_spmv(h, sm, x0, h->r, nullptr, nullptr, 0, nullptr));
+    }
+    init_kernel<<<h->init_grid, 256, 0, sm>>>(h->n, b, x0, x0 ? 1 : 0, h->x, h->r, h->R, h->dinv, h->partials, h->st, h->s, rtol);
+    h->launches++;
+    CK(cudaGetLastError());
+    h->in_solve = true;
+    return 0;
+}
+
+int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
+    if (!h || k_outer < 0) return SSTEP_CG_ERR_ARG;
+    if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "iterate: call solve_begin first");
+    for (int i = 0; i < k_outer; i++) {
+        if (h->use_graph) {
+            CK(cudaGraphLaunch(h->gexec, h->stream));
+            h->launches += kernels_per_outer(h);
+        } else {
+            CK(launch_outer(h, h->stream));
+        }
+        h->graph_launches++;
+    }
+    return 0;
+}
+
+int sstep_cg_solve_end(sstep_cg_t* h, double* x, sstep_cg_result* out) {
+    if (!h) return SSTEP_CG_ERR_ARG;
+    if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "solve_end: call solve_begin first");
+    cudaStream_t sm = h->stream;
+    if (x) CK(cudaMemcpyAsync(x, h->x, sizeof(double) * h->n, cudaMemcpyDeviceToDevice, sm));
+    CK(cudaMemcpyAsync(&h->h_hdr[0], h->st, sizeof(Header), cudaMemcpyDeviceToHost, sm));
+    CK(cudaStreamSynchronize(sm));
+    h->in_solve = false;
+    const Header hd = h->h_hdr[0];
+    const int status = (hd.status == SCG_RUNNING) ? SSTEP_CG_MAXIT : hd.status;
+    if (out) {
+        out->status = status;
+        out->outer_iters = hd.k;
+        out->cg_equiv_iters = (int64_t)hd.k * h->s;
+        out->r0_norm = sqrt(hd.rho0);
+        out->relres = hd.rho0 > 0.0 ? sqrt(hd.rho) / sqrt(hd.rho0) : 0.0;
+        out->solve_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - h->t_begin).count();
+        out->kernel_launches = h->launches;
+    }
+    return status;
+}
+
+int sstep_cg_solve(sstep_cg_t* h, const double* b, const double* x0, double* x, double rtol, int maxit, sstep_cg_result* out) {
+    if (!h || !x || maxit < 0) return SSTEP_CG_ERR_ARG;
+    int rc = sstep_cg_solve_begin(h, b, x0, rtol);
+    if (rc) return rc;
+    cudaStream_t sm = h->stream;
+    // Replay the outer-iteration graph in chunks; two chunks are kept in flight so the device never waits for the
+    // host.  Iterations enqueued after convergence exit on the device flag (a few microseconds each).
+    const int chunk = h->n >= (int64_t(1) << 21) ? 2 : 8;
+    int launched = 0, slot = 0;
+    bool pending[2] = {false, false};
+    bool done = false;
+    while (true) {
+        if (!done && launched < maxit) {
+            const int k = (maxit - launched < chunk) ? maxit - launched : chunk;
+            rc = sstep_cg_iterate(h, k);
+            if (rc) return rc;
+            launched += k;
+            CK(cudaMemcpyAsync(&h->h_hdr[slot], h->st, sizeof(Header), cudaMemcpyDeviceToHost, sm));
+            CK(cudaEventRecord(h->ev[slot], sm));
+            pending[slot] = true;
+            slot ^= 1;
+        }
+        if (pending[slot]) {  // the older of the two chunks
+            CK(cudaEventSynchronize(h->ev[slot]));
+            pending[slot] = false;
+            if (h->h_hdr[slot].status != SCG_RUNNING) done = true;
+        } else if (done || launched >= maxit) {
+            if (pending[slot ^ 1]) {
+                CK(cudaEventSynchronize(h->ev[slot ^ 1]));
+                pending[slot ^ 1] = false;
+            }
+            break;
+        }
+    }
+    return sstep_cg_solve_end(h, x, out);
+}
+
+int sstep_cg_solve_host(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rp, const int32_t* ci, const double* va,
+                        const double* b, const double* x0, double* x, int s, double rtol, int maxit, sstep_cg_result* out) {
+    if (!h || !rp || !ci || !va || !b || !x || n <= 0 || nnz <= 0) return SSTEP_CG_ERR_ARG;
+    CK(cudaSetDevice(h->device));
+    cudaStream_t sm = h->stream;
+    CK(cudaStreamSynchronize(sm));
+    free_problem(h);
+    free_owned(h);
+    CK(cudaMalloc(&h->own_rp, sizeof(int) * (n + 1)));
+    CK(cudaMalloc(&h->own_ci, sizeof(int) * nnz));
+    CK(cudaMalloc(&h->own_va, sizeof(double) * nnz));
+    CK(cudaMalloc(&h->own_b, sizeof(double) * n));
+    CK(cudaMalloc(&h->own_x, sizeof(double) * n));
+    CK(cudaMemcpyAsync(h->own_rp, rp, sizeof(int) * (n + 1), cudaMemcpyHostToDevice, sm));
+    CK(cudaMemcpyAsync(h->own_ci, ci, sizeof(int) * nnz, cudaMemcpyHostToDevice, sm));
+    CK(cudaMemcpyAsync(h->own_va, va, sizeof(double) * nnz, cudaMemcpyHostToDevice, sm));
+    CK(cudaMemcpyAsync(h->own_b, b, sizeof(double) * n, cudaMemcpyHostToDevice, sm));
+    if (x0) CK(cudaMemcpyAsync(h->own_x, x0, sizeof(double) * n, cudaMemcpyHostToDevice, sm));
+    int rc = sstep_cg_setup(h, n, nnz, h->own_rp, h->own_ci, h->own_va, s);
+    if (rc) return rc;
+    rc = sstep_cg_solve(h, h->own_b, x0 ? h->own_x : nullptr, h->own_x, rtol, maxit, out);
+    if (rc < 0) return rc;
+    CK(cudaMemcpyAsync(x, h->own_x, sizeof(double) * n, cudaMemcpyDeviceToHost, sm));
+    CK(cudaStreamSynchronize(sm));
+    return rc;
+}
+
+// ---------------------------------------------------------------- test hooks (production kernels, caller's buffers)
+static int hook_prepare(sstep_cg* h) {
+    if (!h->ready) return fail(h, SSTEP_CG_ERR_STATE, "test hook: call setup first");
+    if (h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "test hook: a solve is in progress");
+    CK(cudaSetDevice(h->device));
+    // st_test: status = running, tickets 0, rho0 = 0 (stop test never fires), rtol = 0
+    ScgState init;
+    memset(&init, 0, sizeof init);
+    init.status = SCG_RUNNING;
+    CK(cudaMemcpyAsync(h->st_test, &init, sizeof(Header) /* header only; tickets stay 0 */, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_spmv(sstep_cg_t* h, const double* x, double* y, double* yjac) {
+    if (!h || !x || !y) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    CK(launch_spmv(h, h->stream, x, y, yjac, nullptr, 0, h->st_test));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_mpk(sstep_cg_t* h, const double* r, double* R, double* AR) {
+    if (!h || !r || !R || !AR) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    // R(:,1) = D^-1 r through the production init kernel (b = r, x0 = 0); x and r outputs go to the workspaces
+    init_kernel<<<h->init_grid, 256, 0, h->stream>>>(h->n, r, nullptr, 0, h->x, h->r, R, h->dinv, h->partials, h->st_test, h->s, 0.0);
+    CK(cudaGetLastError());
+    CK(launch_mpk(h, h->stream, R, AR, h->st_test));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_gram(sstep_cg_t* h, const double* R, const double* AR, const double* AP, const double* r, double* M,
+                       double* C, double* m) {
+    if (!h || !R || !AR || !AP || !r || !M || !C || !m) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    const int s = h->s;
+    CK(launch_gram(h, h->stream, false, R, AR, AP, r, h->st_test, 0));
+    CK(cudaMemcpyAsync(M, h->st_test->M, sizeof(double) * s * s, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(C, h->st_test->C, sizeof(double) * s * s, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaMemcpyAsync(m, h->st_test->m, sizeof(double) * s, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_small_solve(sstep_cg_t* h, const double* M, const double* C, const double* m, const double* Wprev,
+                              double* beta, double* alpha, double* W, int32_t* status_out) {
+    if (!h || !M || !C || !m || !Wprev || !beta || !alpha || !W || !status_out) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    small_solve_kernel<<<1, 32, 0, h->stream>>>(h->s, M, C, m, Wprev, beta, alpha, W, status_out);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_update(sstep_cg_t* h, double* R, const double* AR, double* P, double* AP, double* x, double* r,
+                         const double* beta, const double* alpha, double* rho_out) {
+    if (!h || !R || !AR || !P || !AP || !x || !r || !beta || !alpha) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    CK(launch_update(h, h->stream, false, R, AR, P, AP, x, r, beta, alpha, h->st_test, rho_out));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,195 @@
+// update.cuh -- step a4 (+ the stop test a5): the fused tall-skinny block updates of Alg. 3 l.17-21
+// (PAPER.md:158), every n x s block streamed exactly once (the paper's "Dgemmv" idea):
+//   P  <- R  + P  beta        x <- x + P  alpha
+//   AP <- AR + AP beta        r <- r - AP alpha
+// plus, fused by this build so no extra pass is needed: R(:,1) <- D^-1 r (the next MPK's first column),
+// rho = ||r||^2 with a deterministic single-kernel cross-block finish, k <- k+1 and the stop test
+// ||r|| < rtol ||r_0|| (Alg. 3 l.31-33).
+// Layout: R, AR column-major; P, AP interleaved (one row = s consecutive doubles = 128-bit loads/stores).
+// One thread per row; beta (s x s) and alpha (s) are broadcast from shared memory.
+#pragma once
+#include "common.cuh"
+
+// one half of the update for one row: V <- Xcol + V beta (V = P or AP, interleaved), acc <- acc + sign * (V_new alpha)
+template <int S>
+__device__ __forceinline__ double update_half(int64_t n, int64_t row, const double* __restrict__ Xcm, double* __restrict__ Vil,
+                                              const volatile double* sbeta, const double* salpha, double acc, double sign) {
+    // sbeta is read through a volatile pointer on purpose: it stops the compiler from hoisting all S*S entries into
+    // registers across the row loop (which costs the occupancy this bandwidth-bound kernel lives on)
+    double v[S], out[S];
+    if constexpr (S % 2 == 0) {
+        const double2* v2 = reinterpret_cast<const double2*>(Vil + row * S);
+#pragma unroll
+        for (int l = 0; l < S / 2; l++) {
+            const double2 a = v2[l];
+            v[2 * l] = a.x;
+            v[2 * l + 1] = a.y;
+        }
+    } else {
+#pragma unroll
+        for (int l = 0; l < S; l++) v[l] = Vil[row * S + l];
+    }
+#pragma unroll
+    for (int j = 0; j < S; j++) out[j] = Xcm[(int64_t)j * n + row];
+#pragma unroll
+    for (int j = 0; j < S; j++) {
+        double p = out[j];
+#pragma unroll
+        for (int l = 0; l < S; l++) p = fma(v[l], sbeta[l * S + j], p);
+        out[j] = p;
+        acc = fma(sign * p, salpha[j], acc);
+    }
+    if constexpr (S % 2 == 0) {
+        double2* v2 = reinterpret_cast<double2*>(Vil + row * S);
+#pragma unroll
+        for (int l = 0; l < S / 2; l++) v2[l] = make_double2(out[2 * l], out[2 * l + 1]);
+    } else {
+#pragma unroll
+        for (int l = 0; l < S; l++) Vil[row * S + l] = out[l];
+    }
+    return acc;
+}
+
+template <int S>
+__global__ void __launch_bounds__(256, 2)
+update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
+              double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
+              const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
+              ScgState* __restrict__ st, double* __restrict__ rho_out) {
+    if (st->status != SCG_RUNNING) return;
+    __shared__ double sbeta[S * S];
+    __shared__ double salpha[S];
+    __shared__ double red[8];
+    __shared__ bool is_last;
+    for (int e = threadIdx.x; e < S * S; e += blockDim.x) sbeta[e] = beta_g[e];
+    if (threadIdx.x < S) salpha[threadIdx.x] = alpha_g[threadIdx.x];
+    __syncthreads();
+
+    double rho = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        const double x0 = x[row], r0 = r[row], di = dinv[row];
+        const double xi = update_half<S>(n, row, R, P, sbeta, salpha, x0, 1.0);     // P <- R + P beta ; x += P alpha
+        const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
+        x[row] = xi;
+        r[row] = ri;
+        R[row] = di * ri;  // R(:,1) of the next outer iteration
+        rho = fma(ri, ri, rho);
+    }
+    // ---- ||r||^2: block reduce, per-block partial, ticket, fixed-order finish in the last block ----
+    rho = warp_sum(rho);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = rho;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) v += red[w];
+        partials[blockIdx.x] = v;
+        __threadfence();
+        const unsigned int t = atomicAdd(&st->ticket_update, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    if (threadIdx.x < 32) {
+        __threadfence();
+        double v = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) v += __ldcg(&partials[b]);
+        v = warp_sum(v);
+        if (threadIdx.x == 0) {
+            st->rho = v;
+            st->k = st->k + 1;
+            if (rho_out) rho_out[0] = v;
+            if (!isfinite(v)) st->status = 2;
+            else if (sqrt(v) < st->rtol * sqrt(st->rho0)) st->status = 0;
+            st->ticket_update = 0;
+        }
+    }
+}
+
+// ---- start of a solve: r = b - A x0 (Ax0 already in r if have_ax), x = x0, R(:,1) = D^-1 r, rho0 = ||r||^2 ----
+__global__ void __launch_bounds__(256)
+init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ x0, int have_ax, double* __restrict__ x,
+            double* __restrict__ r, double* __restrict__ R, const double* __restrict__ dinv, double* __restrict__ partials,
+            ScgState* __restrict__ st, int s, double rtol) {
+    __shared__ double red[8];
+    __shared__ bool is_last;
+    double rho = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        const double ri = have_ax ? b[row] - r[row] : b[row];
+        x[row] = x0 ? x0[row] : 0.0;
+        r[row] = ri;
+        R[row] = dinv[row] * ri;
+        rho = fma(ri, ri, rho);
+    }
+    rho = warp_sum(rho);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = rho;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) v += red[w];
+        partials[blockIdx.x] = v;
+        __threadfence();
+        const unsigned int t = atomicAdd(&st->ticket_init, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    if (threadIdx.x < 32) {
+        __threadfence();
+        double v = 0.0;
+        for (int bk = threadIdx.x; bk < (int)gridDim.x; bk += 32) v += __ldcg(&partials[bk]);
+        v = warp_sum(v);
+        for (int e = threadIdx.x; e < s * s; e += 32) {
+            st->W[e] = (e / s == e % s) ? 1.0 : 0.0;  // W_prev = I with C = 0 gives beta = 0, W = M at k = 0
+            st->beta[e] = 0.0;
+        }
+        if (threadIdx.x == 0) {
+            st->rho = v;
+            st->rho0 = v;
+            st->rtol = rtol;
+            st->k = 0;
+            st->status = (v == 0.0) ? 0 : (isfinite(v) ? SCG_RUNNING : 2);
+            st->ticket_init = 0;
+            st->ticket_gram = 0;
+            st->ticket_update = 0;
+        }
+    }
+}
+
+// ---- setup: dinv = 1/a_ii, structural validation, row-length statistics ----
+// err bits: 1 = rowptr not monotone / out of range, 2 = column index out of range, 4 = diagonal missing or <= 0
+__global__ void analyze_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp, const int* __restrict__ ci,
+                               const double* __restrict__ va, double* __restrict__ dinv, int* __restrict__ err,
+                               int* __restrict__ max_len) {
+    const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int e = 0, len = 0;
+    if (row < n) {
+        const int lo = rp[row], hi = rp[row + 1];
+        if (lo < 0 || hi < lo || hi > nnz || (row == 0 && lo != 0) || (row == n - 1 && hi != nnz)) e |= 1;
+        double d = 0.0;
+        bool found = false;
+        if (!e) {
+            len = hi - lo;
+            for (int k = lo; k < hi; k++) {
+                const int c = ci[k];
+                if (c < 0 || c >= n) e |= 2;
+                if (c == row) { d = va[k]; found = true; }
+            }
+            if (!found || !(d > 0.0)) e |= 4;
+        }
+        dinv[row] = (e == 0) ? 1.0 / d : 0.0;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        e |= __shfl_xor_sync(0xffffffffu, e, o);
+        len = max(len, __shfl_xor_sync(0xffffffffu, len, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (e) atomicOr(err, e);
+        atomicMax(max_len, len);
+    }
+}
+
+// Interleave / de-interleave helpers for the Python binding's marshalling are NOT provided: the binding
+// transposes with torch; the kernels only ever see the documented layouts.

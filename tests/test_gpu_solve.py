@@ -1,0 +1,202 @@
+"""End-to-end GPU parity: sstep_cg_solve (graph-captured loop, device-side stop test) against the oracle's
+Alg. 3 (Gram form) on the BASELINE.json configs, at sizes the oracle finishes in seconds, plus the edge and
+degenerate cases.  Bars (north_star): final solution relative difference <= 1e-8, outer iterations within +-1.
+s = 8 with the paper's monomial basis is "parity unpinned" end to end: there the test enforces
+convergence, the true residual and a looser solution bar, and the Chebyshev basis restores the tight bar."""
+import numpy as np
+import pytest
+
+import sstep_inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def cg_mod():
+    import paper_2501_03743_b200 as cg
+    cg.load_library()
+    return cg
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_solve(cg, torch, c, s, rtol, maxit, x0=None, **opts):
+    with cg.SStepCG(0, **opts) as h:
+        h.setup(dev(torch, c["rowptr"]), dev(torch, c["colidx"]), dev(torch, c["vals"]), s)
+        x, res = h.solve(dev(torch, c["b"]), None if x0 is None else dev(torch, x0), rtol=rtol, maxit=maxit)
+        return x.cpu().numpy(), res
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+CASES = [  # cfg, N, s (None = the config's own)
+    (1, 32, None),      # config 1 at full size: 32^3, s=2, rtol 1e-6
+    (1, 32, 1), (1, 32, 3), (1, 32, 4), (1, 32, 5),
+    (2, 48, None),      # config 2 recipe (s=4, 1e-8) at 48^3
+    (3, 24, None),      # config 3 recipe (27-point, s=4) at 24^3
+    (4, 40, 2),         # config 4 recipe at 40^3
+    (5, 20, 4),         # config 5 recipe (variable coefficient, permuted) with s=4
+]
+
+
+@pytest.mark.parametrize("cfg,N,s", CASES)
+def test_solve_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg, N, s):
+    c = gen.make_config(cfg, N=N, s=s)
+    s = c["s"]
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=c["rtol"], maxit=c["maxit"])
+    x, res = gpu_solve(cg_mod, torch_mod, c, s, c["rtol"], c["maxit"])
+    assert ref["status"] == 0 and res["status"] == 0
+    assert abs(res["outer_iters"] - ref["iters"]) <= 1
+    assert res["cg_equiv_iters"] == s * res["outer_iters"]
+    assert res["relres"] < c["rtol"]
+    if res["outer_iters"] != ref["iters"]:     # compare at the oracle's stopping iteration
+        x, res2 = gpu_solve(cg_mod, torch_mod, c, s, 0.0, ref["iters"])
+        assert res2["outer_iters"] == ref["iters"]
+    assert rel(x, ref["x"]) <= 1e-8
+    # and it really solves the system (true residual through the oracle's SpMV)
+    true_res = np.linalg.norm(c["b"] - oracle_mod.spmv(c["rowptr"], c["colidx"], c["vals"], x)) / np.linalg.norm(c["b"])
+    assert true_res <= 2 * c["rtol"]
+
+
+def test_config2_full_size(oracle_mod, cg_mod, torch_mod):
+    """BASELINE.json config 2 at its full size (128^3, n = 2.1M, nnz = 14.6M, s = 4, rtol 1e-8)."""
+    c = gen.make_config(2)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 4, rtol=1e-8, maxit=2000)
+    x, res = gpu_solve(cg_mod, torch_mod, c, 4, 1e-8, 2000)
+    assert ref["status"] == 0 and res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
+    if res["outer_iters"] != ref["iters"]:
+        x, _ = gpu_solve(cg_mod, torch_mod, c, 4, 0.0, ref["iters"])
+    assert rel(x, ref["x"]) <= 1e-8
+    assert rel(x, c["xstar"]) <= 1e-5
+
+
+@pytest.mark.parametrize("cfg,N", [(5, 20), (4, 32)])
+def test_s8_monomial_unpinned_and_chebyshev(oracle_mod, cg_mod, torch_mod, cfg, N):
+    c = gen.make_config(cfg, N=N, s=8)
+    rtol = c["rtol"]
+    x, res = gpu_solve(cg_mod, torch_mod, c, 8, rtol, 2000)
+    assert res["status"] == 0
+    true_res = np.linalg.norm(c["b"] - oracle_mod.spmv(c["rowptr"], c["colidx"], c["vals"], x)) / np.linalg.norm(c["b"])
+    assert true_res <= 2 * rtol
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 8, rtol=rtol, maxit=2000)
+    assert ref["status"] == 0 and rel(x, ref["x"]) <= 1e-4
+    # Chebyshev basis: the tight bars hold again
+    refc = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 8, rtol=rtol, maxit=2000, basis=1)
+    xc, resc = gpu_solve(cg_mod, torch_mod, c, 8, rtol, 2000, basis=1)
+    assert refc["status"] == 0 and resc["status"] == 0 and abs(resc["outer_iters"] - refc["iters"]) <= 1
+    if resc["outer_iters"] != refc["iters"]:
+        xc, _ = gpu_solve(cg_mod, torch_mod, c, 8, 0.0, refc["iters"], basis=1)
+    assert rel(xc, refc["x"]) <= 1e-8
+
+
+def test_iterate_trajectory_matches_oracle(oracle_mod, cg_mod, torch_mod):
+    """solve_begin / iterate(k) / solve_end: iterate i equals the oracle's iterate i (early iterations, s = 3)."""
+    c = gen.make_config(2, N=20)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 3, rtol=0.0, maxit=6, xhist_cap=6, history=True)
+    with cg_mod.SStepCG(0) as h:
+        h.setup(dev(torch_mod, c["rowptr"]), dev(torch_mod, c["colidx"]), dev(torch_mod, c["vals"]), 3)
+        b = dev(torch_mod, c["b"])
+        for k in range(1, 7):
+            h.solve_begin(b, None, 0.0)
+            h.iterate(k)
+            x, res = h.solve_end()
+            assert res["outer_iters"] == k and res["status"] == 1
+            assert rel(x.cpu().numpy(), ref["xhist"][k - 1]) <= 1e-11
+            assert abs(res["relres"] - ref["hist"][k - 1]) <= 1e-9 * ref["hist"][k - 1]
+            assert res["kernel_launches"] == 1 + k * h.get_info("kernels_per_outer")
+
+
+def test_graph_and_direct_launch_agree_bitwise(cg_mod, torch_mod):
+    c = gen.make_config(1, N=24)
+    xs = []
+    for use_graph in (1, 0, 1):
+        x, res = gpu_solve(cg_mod, torch_mod, c, 4, 1e-9, 500, use_graph=use_graph)
+        assert res["status"] == 0
+        xs.append((x, res["outer_iters"]))
+    assert xs[0][1] == xs[1][1] == xs[2][1]
+    assert np.array_equal(xs[0][0], xs[1][0]) and np.array_equal(xs[0][0], xs[2][0])   # deterministic reductions
+
+
+def test_edge_cases(oracle_mod, cg_mod, torch_mod):
+    c = gen.make_config(1, N=10)
+    # x0 != 0 (r0 = b - A x0 through the production SpMV) and x aliasing
+    x0 = np.random.default_rng(9).uniform(-1, 1, c["n"])
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 2, x0=x0, rtol=1e-9, maxit=500)
+    x, res = gpu_solve(cg_mod, torch_mod, c, 2, 1e-9, 500, x0=x0)
+    assert res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1 and rel(x, c["xstar"]) <= 1e-7
+    assert abs(res["r0_norm"] - np.linalg.norm(c["b"] - oracle_mod.spmv(c["rowptr"], c["colidx"], c["vals"], x0))) <= 1e-10
+    # b = 0: converged at once, x = 0, zero iterations
+    cz = dict(c); cz["b"] = np.zeros(c["n"])
+    x, res = gpu_solve(cg_mod, torch_mod, cz, 2, 1e-8, 100)
+    assert res["status"] == 0 and res["outer_iters"] == 0 and np.all(x == 0)
+    # maxit reached -> status 1, x is the last iterate (equals the oracle's)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 2, rtol=1e-14, maxit=3)
+    x, res = gpu_solve(cg_mod, torch_mod, c, 2, 1e-14, 3)
+    assert res["status"] == 1 == ref["status"] and res["outer_iters"] == 3 and rel(x, ref["x"]) <= 1e-12
+    # maxit = 0
+    x, res = gpu_solve(cg_mod, torch_mod, c, 2, 1e-8, 0)
+    assert res["status"] == 1 and res["outer_iters"] == 0 and np.all(x == 0)
+    # s = 16 (SMAX) runs and converges on a well-conditioned system with the Chebyshev basis
+    rp, ci, v, A = gen.random_spd_csr(400, 0.02, 77)
+    cw = dict(rowptr=rp, colidx=ci, vals=v, b=np.random.default_rng(1).uniform(-1, 1, 400), n=400)
+    x, res = gpu_solve(cg_mod, torch_mod, cw, 16, 1e-8, 50, basis=1)
+    assert res["status"] == 0 and rel(x, np.linalg.solve(A, cw["b"])) <= 1e-7
+    # one-row system
+    c1 = dict(rowptr=np.array([0, 1], np.int32), colidx=np.array([0], np.int32), vals=np.array([4.0]), b=np.array([2.0]), n=1)
+    x, res = gpu_solve(cg_mod, torch_mod, c1, 1, 1e-12, 5)
+    assert res["status"] == 0 and abs(x[0] - 0.5) <= 1e-15
+
+
+def test_rank_deficient_block_reports_breakdown(oracle_mod, cg_mod, torch_mod):
+    """Degenerate case of the method (see test_oracle_solvers.test_rank_deficient_last_block)."""
+    rp, ci, v = gen.poisson1d(64)
+    b = np.random.default_rng(22).uniform(-1, 1, 64)
+    c = dict(rowptr=rp, colidx=ci, vals=v, b=b, n=64)
+    ref = oracle_mod.sstep(rp, ci, v, b, 3, rtol=1e-11, maxit=30)
+    x, res = gpu_solve(cg_mod, torch_mod, c, 3, 1e-11, 30)
+    assert ref["status"] == 2 and res["status"] == 2
+    assert abs(res["outer_iters"] - ref["iters"]) <= 1 and np.all(np.isfinite(x))
+
+
+def test_invalid_arguments(cg_mod, torch_mod):
+    rp, ci, v = gen.poisson1d(10)
+    t = lambda a: dev(torch_mod, a)
+    with cg_mod.SStepCG(0) as h:
+        with pytest.raises(cg_mod.SStepCGError):
+            h.setup(t(rp), t(ci), t(v), 0)
+        with pytest.raises(cg_mod.SStepCGError):
+            h.setup(t(rp), t(ci), t(v), 17)
+        bad = v.copy(); bad[0] = -2.0                       # non-positive diagonal
+        with pytest.raises(cg_mod.SStepCGError, match="diagonal"):
+            h.setup(t(rp), t(ci), t(bad), 2)
+        badc = ci.copy(); badc[3] = 99                       # column out of range
+        with pytest.raises(cg_mod.SStepCGError):
+            h.setup(t(rp), t(badc), t(v), 2)
+        with pytest.raises(cg_mod.SStepCGError):             # solve before a successful setup
+            h.solve(t(np.ones(10)))
+        with pytest.raises(cg_mod.SStepCGError):
+            h.set_option("no_such_option", 1)
+        h.setup(t(rp), t(ci), t(v), 2)                       # handle still usable
+        x, res = h.solve(t(np.ones(10)), rtol=1e-12, maxit=10)
+        assert res["status"] == 0
+
+
+def test_solve_host_end_to_end(oracle_mod, cg_mod, torch_mod):
+    c = gen.make_config(1, N=16)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 2, rtol=1e-8, maxit=500)
+    th = lambda a: torch_mod.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    with cg_mod.SStepCG(0) as h:
+        x, res = h.solve_host(th(c["rowptr"]), th(c["colidx"]), th(c["vals"]), th(c["b"]), 2, rtol=1e-8, maxit=500)
+    assert res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
+    assert rel(x.numpy(), ref["x"]) <= 1e-8
