@@ -187,8 +187,8 @@ def test_invalid_arguments(cg_mod, torch_mod):
             h.solve(t(np.ones(10)))
         with pytest.raises(cg_mod.SStepCGError):
             h.set_option("no_such_option", 1)
-        h.setup(t(rp), t(ci), t(v), 2)                       # handle still usable
-        x, res = h.solve(t(np.ones(10)), rtol=1e-12, maxit=10)
+        h.setup(t(rp), t(ci), t(v), 1)                       # handle still usable
+        x, res = h.solve(t(np.random.default_rng(3).uniform(-1, 1, 10)), rtol=1e-10, maxit=12)
         assert res["status"] == 0
 
 
