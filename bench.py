@@ -1,0 +1,411 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of the s-step PCG hot path (BASELINE.json):
+microseconds per OUTER iteration on the 320^3 7-point fp64 Poisson system (config 4), achieved HBM GB/s vs the
+measured peak, GDOF*iter/s; with the CPU oracle timed beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--s 4] [--grid 320] [--sweep 1,2,4,8]
+
+A "step" is one outer iteration (s Jacobi-fused SpMVs, fused Gram + on-device solves, fused block update) replayed
+as one CUDA graph on the live solver state.  Every `restart_every` steps the solve is re-initialised from x0 = 0
+inside the timed region (reading A19 in DESIGN.md: 200 outer iterations at s = 8 would run far past convergence),
+so the timed region holds exactly K outer iterations plus ceil(K/restart_every) cheap re-initialisations.
+Multi-GPU (torchrun): replicas only -- the north_star forbids sharding; every rank runs the same workload and the
+job value aggregates them.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import sstep_inputs as gen  # noqa: E402
+
+METRIC = "sstep_pcg_us_per_outer_iteration"
+NOMINAL_HBM_GBS = 8000.0          # north_star's "~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+# ----------------------------------------------------------------------------------------------- byte model
+def model_bytes(n: int, nnz: int, s: int) -> dict:
+    """Algorithmic (compulsory) HBM bytes of one outer iteration, SURVEY.md §8(d) / DESIGN.md "Byte model"."""
+    csr = 12 * nnz + 4 * (n + 1)
+    mpk = s * csr + 8 * n * (3 * s - 1)       # s matrix sweeps, s gathers + s AR writes + (s-1) R writes
+    gram = 8 * n * (3 * s + 1)                # R, AR, AP blocks + r
+    update = 8 * n * (6 * s + 5)              # 4 block reads, 2 block writes, x, r read+write, R1 write
+    return dict(mpk=mpk, gram=gram, update=update, total=mpk + gram + update, spmv_per_launch=mpk / s)
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def restart_every_for(s: int) -> int:
+    return max(1, 100 // s)       # <= 100 CG-equivalent steps per restart: far from convergence at 320^3
+
+
+# ----------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.idx = device_index
+        self.proc = None
+        self.path = None
+
+    def __enter__(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.idx)], stdout=open(self.path, "w"),
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        try:
+            rows = [ln.split(",") for ln in open(self.path).read().strip().splitlines() if ln.strip()]
+            sm = [float(r[1]) for r in rows]
+            out["samples"] = len(sm)
+            if sm:
+                out["sm_mhz"] = float(np.median(sm))
+                out["sm_max_mhz"] = float(rows[0][2])
+                out["power_w_max"] = max(float(r[3]) for r in rows)
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            for j, nm in enumerate(names):
+                if any(r[5 + j].strip().lower().startswith("active") for r in rows):
+                    out["reasons"].append(nm)
+            os.unlink(self.path)
+        except Exception as e:  # nvidia-smi missing or unparsable: say so instead of inventing numbers
+            out["error"] = str(e)
+        return out
+
+
+# ----------------------------------------------------------------------------------------------- distributed plumbing
+def dist_env():
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return world, rank, local
+
+
+def aggregate_replicas(elapsed_ms: float, k_steps: int, world: int, reduce_max) -> dict:
+    """Job-level numbers of N independent replicas: time = max over ranks, units = all ranks' outer iterations."""
+    t = reduce_max(elapsed_ms)
+    return dict(ms_total=t, ms_per_step=t / k_steps, us_per_outer_job=1e3 * t / (k_steps * world))
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
+    """CUDA-event time (ms) of exactly k_steps outer iterations (graph replays) on the solver's stream."""
+    R = restart_every_for(s)
+    h.solve_begin(b, None, 0.0)
+    h.iterate(warmup)
+    _, res = h.solve_end(want_x=False)
+    assert res["status"] != 2, f"breakdown during warm-up: {res}"
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    ev0.record()
+    done, launches = 0, 0
+    while done < k_steps:
+        k = min(R, k_steps - done)
+        h.solve_begin(b, None, 0.0)
+        h.iterate(k)
+        done += k
+        launches += 1 + k * (s + 2)
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    _, res = h.solve_end(want_x=False)
+    last = k_steps - (k_steps - 1) // R * R
+    assert res["status"] == 1 and res["outer_iters"] == last, f"timed region did not run all iterations: {res}"
+    assert res["relres"] < 1.0, res
+    return ms, launches, res
+
+
+def run_ours(args):
+    import torch
+
+    import paper_2501_03743_b200 as cg
+
+    world, rank, local = dist_env()
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the hot path has no CPU fallback"
+    torch.cuda.set_device(local)
+    reduce_max, barrier = (lambda v: v), (lambda: None)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+        def reduce_max(v):
+            t = torch.tensor([v], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+
+        def barrier():
+            dist.barrier()
+
+    N, s0 = args.grid, args.s
+    t0 = time.time()
+    c = gen.make_config(4, N=N)
+    t_gen = time.time() - t0
+    n, nnz = c["n"], c["nnz"]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda(local)
+    rp, ci, va, b = dev(c["rowptr"]), dev(c["colidx"]), dev(c["vals"]), dev(c["b"])
+    peak, peak_src = measured_peak()
+
+    sweep = {}
+    primary = None
+    s_list = [s0] + [int(t) for t in args.sweep.split(",") if t and int(t) != s0] if args.sweep else [s0]
+    for s in s_list:
+        with cg.SStepCG(local) as h:
+            h.setup(rp, ci, va, s)
+            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid")}
+            if s == s0:
+                with ClockSampler(local) as clk:
+                    ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)
+                clocks = clk.summary()
+            else:
+                ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)
+            agg = aggregate_replicas(ms, args.steps, world, reduce_max)
+            mb = model_bytes(n, nnz, s)
+            us = 1e3 * agg["ms_per_step"]
+            entry = dict(s=s, us_per_outer=us, us_per_cg_equiv_iter=us / s, model_gb_per_outer=mb["total"] / 1e9,
+                         achieved_gbs=mb["total"] / (us * 1e-6) / 1e9,
+                         frac_of_measured_peak=mb["total"] / (us * 1e-6) / 1e9 / peak,
+                         frac_of_nominal_8tbs=mb["total"] / (us * 1e-6) / 1e9 / NOMINAL_HBM_GBS,
+                         gdof_iter_per_s=world * n * s / (us * 1e-6) / 1e9, relres_at_end=res["relres"], **info)
+            # per-kernel device times (un-graphed, CUDA events around every launch, on the live solve state)
+            h.solve_begin(b, None, 0.0)
+            h.iterate(3)
+            reps = max(2, min(10, restart_every_for(s) - 4))
+            t_spmv, t_gram, t_upd = h.profile_outer(reps)
+            h.solve_end(want_x=False)
+            k_us = dict(spmv=1e3 * t_spmv / (reps * s), gram=1e3 * t_gram / reps, update=1e3 * t_upd / reps)
+            entry["kernel_us"] = k_us
+            entry["kernel_gbs"] = dict(spmv=mb["spmv_per_launch"] / k_us["spmv"] / 1e3, gram=mb["gram"] / k_us["gram"] / 1e3,
+                                       update=mb["update"] / k_us["update"] / 1e3)
+            entry["kernel_frac_of_measured_peak"] = {k: v / peak for k, v in entry["kernel_gbs"].items()}
+            entry["kernel_share_of_step"] = {k: (v * (s if k == "spmv" else 1)) / (s * k_us["spmv"] + k_us["gram"] + k_us["update"])
+                                             for k, v in k_us.items()}
+            sweep[str(s)] = entry
+            if s == s0:
+                primary = dict(entry, launches=launches, agg=agg, mb=mb)
+    return dict(world=world, rank=rank, local=local, c=c, n=n, nnz=nnz, N=N, sweep=sweep, primary=primary, clocks=clocks,
+                peak=peak, peak_src=peak_src, t_gen=t_gen, dev=(rp, ci, va, b))
+
+
+def run_e2e(args, ctx):
+    """The same metric through the C-ABI call with HOST buffers: H2D of CSR + b, setup, k outer iterations,
+    D2H of x, all inside the timed region."""
+    import torch
+
+    import paper_2501_03743_b200 as cg
+    c, s = ctx["c"], args.s
+    k = min(args.steps, restart_every_for(s))
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    rp, ci, va, b = pin(c["rowptr"]), pin(c["colidx"]), pin(c["vals"]), pin(c["b"])
+    x = torch.empty(c["n"], dtype=torch.float64).pin_memory()
+    best = None
+    with cg.SStepCG(ctx["local"]) as h:
+        for _ in range(2):  # first pass warms allocator / graph instantiation paths; report the second
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ev0.record()
+            _, res = h.solve_host(rp, ci, va, b, s, rtol=0.0, maxit=k, x_out=x)
+            ev1.record()
+            torch.cuda.synchronize()
+            wall_ms = 1e3 * (time.perf_counter() - t0)
+            best = dict(ms=max(ev0.elapsed_time(ev1), wall_ms), res=res)
+    assert best["res"]["outer_iters"] == k and best["res"]["status"] == 1
+    h2d = rp.numel() * 4 + ci.numel() * 4 + va.numel() * 8 + b.numel() * 8
+    return dict(value=1e3 * best["ms"] / k, unit="us", h2d_bytes_per_step=h2d / k, d2h_bytes_per_step=x.numel() * 8 / k,
+                outer_iters=k, note="one sstep_cg_solve_host call: pinned host CSR+b -> device, setup (dinv, graph capture), "
+                                    f"{k} outer iterations, x -> host; all inside the timed region")
+
+
+def run_cpu_baseline(args, ctx):
+    """The oracle as it stands, on the host cores of this box, on a bounded sample of the same workload."""
+    import oracle
+    c, s = ctx["c"], args.s
+    iters = 2
+    t0 = time.perf_counter()
+    ref = oracle.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=0.0, maxit=iters)
+    dt = time.perf_counter() - t0
+    assert ref["iters"] == iters
+    return dict(value=1e6 * dt / iters, unit="us", cores=1, kind="oracle",
+                sample=f"first {iters} outer iterations (s={s}) of the same {ctx['N']}^3 system at full size, single thread, "
+                       f"including the oracle's own start-up (dinv, r0)", seconds=dt)
+
+
+# ----------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """--impl reference: the oracle (oracle/sstep_oracle.c, as it stands, single thread) on this box's host cores.
+    A step is ONE oracle outer iteration on a bounded sample of config 4: the 7-point operator on a
+    grid x grid x nz z-slab (same plane size, same nnz/row), nz sized so that warm-up + K steps end within
+    ~2.5 minutes; the reported value is scaled by grid/nz to the rows of the full workload."""
+    import oracle
+    world, rank, _ = dist_env()
+    if rank != 0:
+        return None
+    N, s, K, W = args.grid, args.s, args.steps, args.warmup
+    R = restart_every_for(s)
+
+    def slab(nz):
+        rp, ci, va = gen.poisson7_box(N, N, nz)
+        xs = np.random.default_rng(3).uniform(-1.0, 1.0, N * N * nz)
+        return rp, ci, va, gen.apply_poisson7_box(N, N, nz, xs)
+
+    rp, ci, va, b = slab(4)
+    t0 = time.perf_counter()
+    oracle.sstep(rp, ci, va, b, s, rtol=0.0, maxit=2)
+    per_row = (time.perf_counter() - t0) / 2 / (N * N * 4)
+    budget = float(os.environ.get("SSTEP_REF_BUDGET_S", "150"))
+    nz = int(max(2, min(N, budget / ((K + W) * per_row * N * N))))
+    rp, ci, va, b = slab(nz)
+
+    def run(k):
+        done, t = 0, 0.0
+        while done < k:
+            kk = min(R, k - done)
+            t0 = time.perf_counter()
+            res = oracle.sstep(rp, ci, va, b, s, rtol=0.0, maxit=kk)
+            t += time.perf_counter() - t0
+            assert res["iters"] == kk and res["status"] == 1, res
+            done += kk
+        return t
+
+    run(W)
+    t = run(K)
+    us_sample = 1e6 * t / K
+    us_full = us_sample * N / nz
+    n, nnz = N ** 3, 7 * N ** 3 - 6 * N ** 2
+    sample = (f"{K} oracle outer iterations (s={s}) on the {N}x{N}x{nz} z-slab of the {N}^3 7-point system, single thread, "
+              f"restarted from x0=0 every {R} iterations; value scaled by {N}/{nz} to the full row count")
+    return {
+        "metric": METRIC, "value": us_full, "unit": "us", "n_gpus": args.gpus, "steps": K, "warmup": W,
+        "ms_per_step": us_full / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "impl": "reference",
+        "config": {"workload": f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, Jacobi, s={s}",
+                   "s": s, "sample": sample},
+        "cpu_baseline": {"value": us_full, "unit": "us", "cores": 1, "kind": "oracle", "sample": sample,
+                         "measured_us_per_step_on_sample": us_sample},
+        "e2e": {"value": us_full, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+        "gdof_iter_per_s": n * s / (us_full * 1e-6) / 1e9,
+    }
+
+
+# ----------------------------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)       # config 4: "fixed 200 outer iterations for timing"
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--s", type=int, default=4, help="block size of the headline value (paper uses s <= 5)")
+    ap.add_argument("--grid", type=int, default=320, help="grid edge N of config 4 (N^3 unknowns)")
+    ap.add_argument("--sweep", type=str, default="1,2,4,8", help="block sizes also reported (config 4's sweep); '' = none")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        line = run_reference(args)
+        if line is not None:
+            print(json.dumps(line), flush=True)
+        return
+
+    ctx = run_ours(args)
+    world, rank = ctx["world"], ctx["rank"]
+    if world != args.gpus and rank == 0:
+        print(f"[bench] note: --gpus {args.gpus} but WORLD_SIZE={world}; reporting n_gpus={world}", file=sys.stderr)
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(args, ctx)          # every rank runs it (replicas); rank 0 reports its own
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = run_cpu_baseline(args, ctx)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    p, s, N, n, nnz = ctx["primary"], args.s, ctx["N"], ctx["n"], ctx["nnz"]
+    mb = p["mb"]
+    k_us = p["kernel_us"]["spmv"]
+    line = {
+        "metric": METRIC,
+        "value": p["agg"]["us_per_outer_job"],
+        "unit": "us",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": p["agg"]["ms_per_step"],
+        "higher_is_better": False,
+        "scaling": "weak",
+        "vs_baseline": None,             # BASELINE.md holds no published number for this metric/workload
+        "dtype": "f64",
+        "data": "synthetic",
+        "config": {
+            "workload": f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, b=A x*, x*~U[-1,1] seed 3, "
+                        f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)",
+            "s": s, "grid": N, "restart_every": restart_every_for(s),
+            "l2": "inputs larger than L2: one outer iteration streams %.1f GB >> 126 MB" % (mb["total"] / 1e9),
+            "parallelism": "replicas only (north_star: one GPU, no sharding)" if world > 1 else "single GPU",
+        },
+        "gdof_iter_per_s": p["gdof_iter_per_s"],
+        "achieved_gbs": p["achieved_gbs"],
+        "iteration_roofline": {"bound": "hbm", "achieved": p["achieved_gbs"], "peak": ctx["peak"], "unit": "GB/s",
+                               "frac": p["frac_of_measured_peak"], "frac_of_nominal_8tbs": p["frac_of_nominal_8tbs"],
+                               "algorithmic_bytes_per_outer": mb["total"]},
+        "roofline": {"bound": "hbm", "kernel": "spmv_bulk_kernel (Jacobi-fused CSR SpMV, s launches per outer iteration)"
+                     if p["spmv_bulk"] else "spmv_vec_kernel",
+                     "achieved": mb["spmv_per_launch"] / k_us / 1e3, "peak": ctx["peak"], "unit": "GB/s",
+                     "frac": mb["spmv_per_launch"] / k_us / 1e3 / ctx["peak"], "peak_source": ctx["peak_src"],
+                     "algorithmic_bytes_per_launch": mb["spmv_per_launch"], "avg_launch_us": k_us,
+                     "share_of_step": p["kernel_share_of_step"]["spmv"],
+                     "traffic": None},
+        "kernels": {"us": p["kernel_us"], "gbs": p["kernel_gbs"], "frac_of_measured_peak": p["kernel_frac_of_measured_peak"],
+                    "share_of_step": p["kernel_share_of_step"]},
+        "sweep": ctx["sweep"],
+        "clocks": ctx["clocks"],
+        "gpu_launches": p["launches"],
+        "e2e": e2e,
+        "cpu_baseline": cpu,
+        "host_generation_seconds": ctx["t_gen"],
+    }
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

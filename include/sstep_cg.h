@@ -117,6 +117,13 @@ int sstep_cg_solve_host(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_
                         const double *x0_host, double *x_host, int s, double rtol, int maxit,
                         sstep_cg_result *out);
 
+/* Measurement aid (bench.py's `roofline` object).  Between solve_begin and solve_end: run `reps` outer
+ * iterations on the live solve state with the kernels launched one by one (no graph) and a CUDA event pair
+ * around every launch on the solver's stream.  ms_host[0] = summed device milliseconds of the s*reps SpMV
+ * launches, ms_host[1] = of the reps Gram+solve launches, ms_host[2] = of the reps update launches.
+ * Synchronises the stream.  The iterations count as real ones (x, r, k advance). */
+int sstep_cg_profile_outer(sstep_cg_t *handle, int reps, double *ms_host);
+
 int sstep_cg_destroy(sstep_cg_t *handle);
 
 /* Text of the last failure on this handle ("" if none).  Never NULL. */

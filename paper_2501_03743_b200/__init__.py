@@ -22,7 +22,7 @@ SMAX = 16
 STATUS_NAMES = {0: "converged", 1: "maxit", 2: "breakdown"}
 EXPORTED_SYMBOLS = [
     "sstep_cg_create", "sstep_cg_setup", "sstep_cg_set_option", "sstep_cg_get_info", "sstep_cg_solve",
-    "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_solve_host", "sstep_cg_destroy",
+    "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_profile_outer", "sstep_cg_solve_host", "sstep_cg_destroy",
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update",
 ]
@@ -65,6 +65,7 @@ def load_library(build: bool = True):
     lib.sstep_cg_solve_begin.argtypes = [vp, vp, vp, dbl]
     lib.sstep_cg_iterate.argtypes = [vp, i32]
     lib.sstep_cg_solve_end.argtypes = [vp, vp, C.POINTER(_Result)]
+    lib.sstep_cg_profile_outer.argtypes = [vp, i32, C.POINTER(dbl)]
     lib.sstep_cg_solve_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, dbl, i32, C.POINTER(_Result)]
     lib.sstep_cg_destroy.argtypes = [vp]
     lib.sstep_cg_last_error.argtypes = [vp]
@@ -184,6 +185,12 @@ class SStepCG:
 
     def iterate(self, k_outer: int):
         self._check(self._lib.sstep_cg_iterate(self._h, int(k_outer)), "sstep_cg_iterate")
+
+    def profile_outer(self, reps: int):
+        """Per-kernel-class device milliseconds of `reps` un-graphed outer iterations: (spmv, gram, update)."""
+        ms = (C.c_double * 3)()
+        self._check(self._lib.sstep_cg_profile_outer(self._h, int(reps), ms), "sstep_cg_profile_outer")
+        return float(ms[0]), float(ms[1]), float(ms[2])
 
     def solve_end(self, want_x: bool = True):
         torch = _torch()

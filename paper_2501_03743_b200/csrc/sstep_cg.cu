@@ -487,6 +487,59 @@ int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
     return 0;
 }
 
+int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
+    if (!h || reps < 1 || !ms_host) return SSTEP_CG_ERR_ARG;
+    if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "profile_outer: call solve_begin first");
+    cudaStream_t sm = h->stream;
+    const int per = h->s + 2;
+    const int nev = reps * per * 2;
+    cudaEvent_t* evs = new cudaEvent_t[nev];
+    for (int i = 0; i < nev; i++) evs[i] = nullptr;
+    int rc = 0;
+    auto body = [&]() -> int {
+        for (int i = 0; i < nev; i++) CK(cudaEventCreate(&evs[i]));
+        int e = 0;
+        const int64_t n = h->n;
+        for (int rep = 0; rep < reps; rep++) {
+            for (int j = 0; j < h->s; j++) {
+                double* yjac = (j + 1 < h->s) ? h->R + (int64_t)(j + 1) * n : nullptr;
+                int mode = 0;
+                const double* xprev = nullptr;
+                if (h->basis == SSTEP_CG_BASIS_CHEBYSHEV) {
+                    mode = (j == 0) ? 1 : 2;
+                    if (j > 0) xprev = h->R + (int64_t)(j - 1) * n;
+                }
+                CK(cudaEventRecord(evs[e++], sm));
+                CK(launch_spmv(h, sm, h->R + (int64_t)j * n, h->AR + (int64_t)j * n, yjac, xprev, mode, h->st));
+                CK(cudaEventRecord(evs[e++], sm));
+            }
+            CK(cudaEventRecord(evs[e++], sm));
+            CK(launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1));
+            CK(cudaEventRecord(evs[e++], sm));
+            CK(cudaEventRecord(evs[e++], sm));
+            CK(launch_update(h, sm, false, h->R, h->AR, h->P, h->AP, h->x, h->r, h->st->beta, h->st->alpha, h->st, nullptr));
+            CK(cudaEventRecord(evs[e++], sm));
+            h->graph_launches++;
+        }
+        CK(cudaStreamSynchronize(sm));
+        ms_host[0] = ms_host[1] = ms_host[2] = 0.0;
+        e = 0;
+        for (int rep = 0; rep < reps; rep++)
+            for (int k = 0; k < per; k++) {
+                float ms = 0.f;
+                CK(cudaEventElapsedTime(&ms, evs[e], evs[e + 1]));
+                e += 2;
+                ms_host[k < h->s ? 0 : (k == h->s ? 1 : 2)] += ms;
+            }
+        return 0;
+    };
+    rc = body();
+    for (int i = 0; i < nev; i++)
+        if (evs[i]) cudaEventDestroy(evs[i]);
+    delete[] evs;
+    return rc;
+}
+
 int sstep_cg_solve_end(sstep_cg_t* h, double* x, sstep_cg_result* out) {
     if (!h) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "solve_end: call solve_begin first");

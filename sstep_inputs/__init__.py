@@ -21,7 +21,7 @@ from __future__ import annotations
 import numpy as np
 
 __all__ = [
-    "poisson7", "poisson27", "varcoef7", "apply_poisson7", "apply_poisson27",
+    "poisson7", "poisson7_box", "apply_poisson7_box", "poisson27", "varcoef7", "varcoef_cells", "apply_poisson7", "apply_poisson27",
     "apply_varcoef7", "symmetric_permute", "random_spd_csr", "poisson1d",
     "make_config", "CONFIG_NAMES",
 ]
@@ -30,37 +30,39 @@ __all__ = [
 # --------------------------------------------------------------------------
 # constant-coefficient stencils
 # --------------------------------------------------------------------------
-def _grid_coords(N: int, z0: int, z1: int):
-    """x, y, z coordinates (int32) of the rows in the z-slab [z0, z1)."""
+def _grid_coords(N, z0: int, z1: int):
+    """x, y, z coordinates (int32) of the rows in the z-slab [z0, z1); N is an int (cube) or (nx, ny, nz)."""
+    nx, ny, _ = (N, N, N) if isinstance(N, int) else N
     zz, yy, xx = np.meshgrid(np.arange(z0, z1, dtype=np.int32),
-                             np.arange(N, dtype=np.int32),
-                             np.arange(N, dtype=np.int32), indexing="ij")
+                             np.arange(ny, dtype=np.int32),
+                             np.arange(nx, dtype=np.int32), indexing="ij")
     return xx.ravel(), yy.ravel(), zz.ravel()
 
 
-def _stencil_csr(N: int, offsets, diag_value: float, off_value: float, slab: int = 16):
-    """CSR of a constant-coefficient stencil on an N^3 grid with homogeneous
-    Dirichlet boundaries (neighbours outside the cube are dropped).
+def _stencil_csr(N, offsets, diag_value: float, off_value: float, slab: int = 16):
+    """CSR of a constant-coefficient stencil on an N^3 grid (or an (nx, ny, nz) box) with homogeneous
+    Dirichlet boundaries (neighbours outside the box are dropped).
 
     `offsets` is a list of (dx, dy, dz) in ascending column order.
     Built slab by slab in z to bound the temporary memory.
     """
-    n = N * N * N
+    nx, ny, nz = (N, N, N) if isinstance(N, int) else N
+    n = nx * ny * nz
     counts = np.empty(n, dtype=np.int32)
     col_parts, val_parts = [], []
-    for z0 in range(0, N, slab):
-        z1 = min(N, z0 + slab)
-        x, y, z = _grid_coords(N, z0, z1)
-        rows = x.astype(np.int64) + N * (y.astype(np.int64) + N * z.astype(np.int64))
+    for z0 in range(0, nz, slab):
+        z1 = min(nz, z0 + slab)
+        x, y, z = _grid_coords((nx, ny, nz), z0, z1)
+        rows = x.astype(np.int64) + nx * (y.astype(np.int64) + ny * z.astype(np.int64))
         m = rows.size
         cols = np.empty((m, len(offsets)), dtype=np.int32)
         mask = np.empty((m, len(offsets)), dtype=bool)
         vals = np.empty((m, len(offsets)), dtype=np.float64)
         for k, (dx, dy, dz) in enumerate(offsets):
-            ok = ((x + dx >= 0) & (x + dx < N) & (y + dy >= 0) & (y + dy < N)
-                  & (z + dz >= 0) & (z + dz < N))
+            ok = ((x + dx >= 0) & (x + dx < nx) & (y + dy >= 0) & (y + dy < ny)
+                  & (z + dz >= 0) & (z + dz < nz))
             mask[:, k] = ok
-            cols[:, k] = (rows + dx + N * (dy + N * dz)).astype(np.int32)
+            cols[:, k] = (rows + dx + nx * (dy + ny * dz)).astype(np.int32)
             vals[:, k] = diag_value if (dx == 0 and dy == 0 and dz == 0) else off_value
         counts[rows[0]:rows[0] + m] = mask.sum(axis=1)
         col_parts.append(cols[mask])
@@ -80,6 +82,24 @@ def poisson7(N: int):
     Dirichlet (BASELINE.json configs 1, 2, 4; PAPER.md:259 — the paper says
     "five-point", its 514-iteration count fixes the 7-point stencil)."""
     return _stencil_csr(N, _OFF7, 6.0, -1.0)
+
+
+def poisson7_box(nx: int, ny: int, nz: int):
+    """The same 7-point operator on an nx x ny x nz box: a z-slab of the cube keeps the plane size and the
+    nnz/row of the full problem (used for bounded CPU-baseline samples of config 4)."""
+    return _stencil_csr((nx, ny, nz), _OFF7, 6.0, -1.0)
+
+
+def apply_poisson7_box(nx: int, ny: int, nz: int, x: np.ndarray) -> np.ndarray:
+    u = x.reshape(nz, ny, nx)
+    out = 6.0 * u
+    out[1:, :, :] -= u[:-1, :, :]
+    out[:-1, :, :] -= u[1:, :, :]
+    out[:, 1:, :] -= u[:, :-1, :]
+    out[:, :-1, :] -= u[:, 1:, :]
+    out[:, :, 1:] -= u[:, :, :-1]
+    out[:, :, :-1] -= u[:, :, 1:]
+    return out.ravel()
 
 
 def poisson27(N: int):

@@ -107,3 +107,18 @@ def test_configs_are_seeded_and_consistent():
     assert c5["s"] == 8 and c5["nnz"] == 7 * 125 - 6 * 25
     c6 = gen.make_config(6, N=5)
     assert np.all(c6["b"] == 1.0) and c6["rtol"] == 1e-6
+
+
+def test_poisson7_box_matches_cube_and_definition():
+    rp, ci, v = gen.poisson7_box(5, 5, 5)
+    rp7, ci7, v7 = gen.poisson7(5)
+    assert np.array_equal(rp, rp7) and np.array_equal(ci, ci7) and np.array_equal(v, v7)
+    nx, ny, nz = 6, 4, 3
+    A = _dense(*gen.poisson7_box(nx, ny, nz))
+    assert np.array_equal(A, A.T) and A.shape[0] == nx * ny * nz
+    x = np.random.default_rng(2).uniform(-1, 1, nx * ny * nz)
+    assert np.allclose(A @ x, gen.apply_poisson7_box(nx, ny, nz, x), rtol=0, atol=1e-13)
+    kx, ky, kz = (np.arange(1, m + 1) for m in (nx, ny, nz))
+    lam = (6 - 2 * (np.cos(kz * np.pi / (nz + 1))[:, None, None] + np.cos(ky * np.pi / (ny + 1))[None, :, None]
+                    + np.cos(kx * np.pi / (nx + 1))[None, None, :])).ravel()
+    assert np.allclose(np.sort(np.linalg.eigvalsh(A)), np.sort(lam), atol=1e-12)
