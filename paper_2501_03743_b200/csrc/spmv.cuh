@@ -8,6 +8,8 @@
 //   spmv_bulk_kernel : per-warp multi-stage pipeline; the warp's slice of colidx/vals is streamed into
 //                      shared memory by the TMA engine (cp.async.bulk, 16 B aligned, L2 evict-first) while the
 //                      warp gathers x for the previous tile.  Needs every tile of 32/L rows to hold < CAP-3 nnz.
+// 1/a_ii: the bulk kernel takes it from the row's own diagonal entry (__drcp_rn = the IEEE quotient 1/a_ii, the same
+// bits as the dinv array the generic kernel reads).
 #pragma once
 #include "common.cuh"
 
@@ -52,16 +54,27 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
 // Tile t covers rows [t*RPT, (t+1)*RPT), RPT = 32/L; its nnz range [rp[row0], rp[row1]) is copied from the
 // 16 B aligned element a0 = rp[row0] & ~3 on.  Tiles are dealt to warps round-robin so that at any time the
 // grid works on one contiguous window of rows (keeps the gathered vector's working set in L2/L1).
+//
+// Per tile a lane holds a register fragment: its first U entries of the row (values, gathered x), the row's
+// diagonal entry a_ii (1/a_ii is taken from the row itself: no dinv array is read) and the
+// partial sum of any entries beyond U*L (long rows, summed when the fragment is loaded).  Once the fragment is in
+// registers the slot is free and the copy of the warp's tile i+D is issued into it.  (Loading the fragment of tile
+// i+1 before tile i is reduced was measured slower: it doubles the registers and halves the resident warps.)
+template <int U>
+struct SpmvFrag {
+    double v[U], xv[U];
+    double diag, rem, xrow, xprev;
+};
+
 template <int L, int D, int CAP, int WPC>
-__global__ void __launch_bounds__(WPC * 32) spmv_bulk_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp,
+__global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp,
                                                              const int* __restrict__ ci, const double* __restrict__ va,
-                                                             const double* __restrict__ dinv, const double* __restrict__ x,
-                                                             double* __restrict__ y, double* __restrict__ yjac,
-                                                             const double* __restrict__ xprev, int mode,
-                                                             const ScgState* __restrict__ st, int64_t num_tiles) {
+                                                             const double* __restrict__ x, double* __restrict__ y,
+                                                             double* __restrict__ yjac, const double* __restrict__ xprev,
+                                                             int mode, const ScgState* __restrict__ st, int64_t num_tiles) {
     if (st && st->status != SCG_RUNNING) return;
     constexpr int RPT = 32 / L;
-    constexpr int U = (L == 1) ? 8 : 4;  // predicated unroll of the gather loop
+    constexpr int U = 8;  // entries per lane held in registers (rows up to 8 L entries need no remainder loop)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     double* svals = reinterpret_cast<double*>(smem_raw) + (size_t)warp * D * CAP;
@@ -79,6 +92,8 @@ __global__ void __launch_bounds__(WPC * 32) spmv_bulk_kernel(int64_t n, int64_t 
     const int64_t gw = (int64_t)blockIdx.x * WPC + warp;
     if (gw >= num_tiles) return;
     const int64_t my_tiles = (num_tiles - gw + GW - 1) / GW;
+    const int g = lane % L;
+    const bool jac = yjac != nullptr;
 
     // issue the copies of this warp's i-th tile into slot i % D; nz0/nz1 = its nnz range (valid in lane 0)
     auto issue = [&](int64_t i, int nz0, int nz1) {
@@ -118,60 +133,94 @@ __global__ void __launch_bounds__(WPC * 32) spmv_bulk_kernel(int64_t n, int64_t 
         nz0 = rp[row0];
         nz1 = rp[row1];
     };
+    auto row_of = [&](int64_t i) { return (gw + i * GW) * RPT + lane / L; };
 
-    // prologue: fill D-1 slots
-    int nb0 = 0, nb1 = 0;  // bounds of the next tile to issue (prefetched one iteration ahead)
-    for (int64_t i = 0; i < D - 1 && i < my_tiles; i++) {
-        int a = 0, b = 0;
-        if (lane == 0) tile_bounds(i, a, b);
-        issue(i, a, b);
-    }
-    if (lane == 0 && D - 1 < my_tiles) tile_bounds(D - 1, nb0, nb1);
-    // per-row bounds of the first tile
-    const int g = lane % L;
-    int lo_n = 0, hi_n = 0;
-    {
-        const int64_t row = gw * RPT + lane / L;
-        if (row < n) { lo_n = rp[row]; hi_n = rp[row + 1]; }
-    }
-    for (int64_t i = 0; i < my_tiles; i++) {
-        const int64_t t = gw + i * GW;
-        const int64_t row = t * RPT + lane / L;
-        const int lo = lo_n, hi = hi_n;
-        // prefetch: per-row bounds of tile i+1, nnz range of tile i+D; issue tile i+D-1 into the slot freed last
-        if (i + 1 < my_tiles) {
-            const int64_t rown = row + GW * RPT;
-            lo_n = hi_n = 0;
-            if (rown < n) { lo_n = rp[rown]; hi_n = rp[rown + 1]; }
-        }
-        if (i + D - 1 < my_tiles) {
-            issue(i + D - 1, nb0, nb1);
-            if (lane == 0 && i + D < my_tiles) tile_bounds(i + D, nb0, nb1);
-        }
+    // slot i % D -> registers (waits for the copy; reads this lane's entries; issues the x gather)
+    auto load_frag = [&](int64_t i, int lo, int hi, SpmvFrag<U>& f) {
         const int sl = (int)(i % D);
+        const int64_t row = row_of(i);
         const int a0 = __shfl_sync(0xffffffffu, lo, 0) & ~3;
         mbar_wait(&bars[sl], (uint32_t)((i / D) & 1));
         const double* sv = svals + sl * CAP - a0;
         const int* sc = scols + sl * CAP - a0;
-        double acc = 0.0;
-        for (int k = lo + g; k < hi; k += U * L) {
-            int c[U];
-            double v[U], xv[U];
+        int c[U];
+        f.diag = 0.0;
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const int kk = k + u * L;
-                const bool ok = kk < hi;
-                c[u] = ok ? sc[kk] : -1;
-                v[u] = ok ? sv[kk] : 0.0;
-            }
-#pragma unroll
-            for (int u = 0; u < U; u++) xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
-#pragma unroll
-            for (int u = 0; u < U; u++) acc = fma(v[u], xv[u], acc);
+        for (int u = 0; u < U; u++) {
+            const int kk = lo + g + u * L;
+            const bool ok = kk < hi;
+            c[u] = ok ? sc[kk] : -1;
+            f.v[u] = ok ? sv[kk] : 0.0;
+            if (c[u] == row) f.diag = f.v[u];
         }
+#pragma unroll
+        for (int u = 0; u < U; u++) f.xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
+        f.xrow = 0.0;
+        f.xprev = 0.0;
+        if (jac && mode != 0 && row < n) {
+            f.xrow = x[row];
+            if (mode == 2) f.xprev = xprev[row];
+        }
+        double rem = 0.0;
+        for (int k = lo + g + U * L; k < hi; k += L) {  // long rows only
+            const int cc = sc[k];
+            const double vv = sv[k];
+            if (cc == row) f.diag = vv;
+            rem = fma(vv, x[cc], rem);
+        }
+        f.rem = rem;
+        __syncwarp();  // every lane has read the slot: it may be refilled
+    };
+    auto finish = [&](int64_t i, const SpmvFrag<U>& f) {
+        const int64_t row = row_of(i);
+        double acc = 0.0;
+#pragma unroll
+        for (int u = 0; u < U; u++) acc = fma(f.v[u], f.xv[u], acc);
+        acc += f.rem;
         acc = group_sum<L>(acc);
-        if (g == 0 && row < n) spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
-        __syncwarp();
+        double d = f.diag;
+        if (L > 1 && jac) d = group_sum<L>(d);  // exactly one lane of the group holds a_ii, the others 0
+        if (g == 0 && row < n) {
+            y[row] = acc;
+            if (jac) {
+                double z = __drcp_rn(d) * acc;  // = (1 / a_ii) * acc, the same two roundings as a dinv array
+                if (mode == 1) z = z - f.xrow;
+                else if (mode == 2) z = 2.0 * (z - f.xrow) - f.xprev;
+                yjac[row] = z;
+            }
+        }
+    };
+    auto row_bounds = [&](int64_t i, int& lo, int& hi) {
+        lo = hi = 0;
+        if (i < my_tiles) {
+            const int64_t row = row_of(i);
+            if (row < n) { lo = rp[row]; hi = rp[row + 1]; }
+        }
+    };
+
+    // prologue: fill the ring
+    int nb0 = 0, nb1 = 0;  // nnz range of the next tile to issue (lane 0; fetched one step ahead)
+    for (int64_t i = 0; i < D && i < my_tiles; i++) {
+        int a = 0, b = 0;
+        if (lane == 0) tile_bounds(i, a, b);
+        issue(i, a, b);
+    }
+    if (lane == 0 && D < my_tiles) tile_bounds(D, nb0, nb1);
+    int lo_n, hi_n;  // per-row bounds of the next fragment to load (fetched one step ahead)
+
+    {
+        SpmvFrag<U> cur;
+        row_bounds(0, lo_n, hi_n);
+        for (int64_t i = 0; i < my_tiles; i++) {
+            const int lo = lo_n, hi = hi_n;
+            row_bounds(i + 1, lo_n, hi_n);
+            load_frag(i, lo, hi, cur);
+            if (i + D < my_tiles) {
+                issue(i + D, nb0, nb1);
+                if (lane == 0 && i + D + 1 < my_tiles) tile_bounds(i + D + 1, nb0, nb1);
+            }
+            finish(i, cur);
+        }
     }
 }
 

@@ -19,8 +19,8 @@ struct Header {  // mirrors the first fields of ScgState
     double rho, rho0, rtol;
 };
 
-constexpr int BULK_D = 3, BULK_CAP = 256, BULK_WPC = 8;
-constexpr size_t BULK_SMEM = (size_t)BULK_WPC * BULK_D * BULK_CAP * 12 + (size_t)BULK_WPC * BULK_D * 8;
+constexpr int BULK_CAP = 256, BULK_WPC = 8;
+constexpr size_t bulk_smem(int D) { return (size_t)BULK_WPC * D * BULK_CAP * 12 + (size_t)BULK_WPC * D * 8; }
 
 }  // namespace
 
@@ -30,7 +30,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -81,12 +81,24 @@ int fail(sstep_cg* h, int code, const std::string& msg) {
     } while (0)
 
 // ---------------------------------------------------------------- kernel dispatch
+using bulk_fn_t = void (*)(int64_t, int64_t, const int*, const int*, const double*, const double*, double*, double*,
+                           const double*, int, const ScgState*, int64_t);
+
+template <int L>
+bulk_fn_t bulk_kernel_for(int depth) {
+    switch (depth) {
+        case 2: return spmv_bulk_kernel<L, 2, BULK_CAP, BULK_WPC>;
+        case 3: return spmv_bulk_kernel<L, 3, BULK_CAP, BULK_WPC>;
+        default: return spmv_bulk_kernel<L, 4, BULK_CAP, BULK_WPC>;
+    }
+}
+
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st) {
     if (h->bulk) {
-        spmv_bulk_kernel<L, BULK_D, BULK_CAP, BULK_WPC><<<h->spmv_grid, BULK_WPC * 32, BULK_SMEM, sm>>>(
-            h->n, h->nnz, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, h->num_tiles);
+        bulk_kernel_for<L>(h->spmv_depth)<<<h->spmv_grid, BULK_WPC * 32, bulk_smem(h->spmv_depth), sm>>>(
+            h->n, h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->num_tiles);
     } else {
         spmv_vec_kernel<L><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st);
     }
@@ -111,10 +123,11 @@ cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
     if (h->bulk) {
-        auto k = spmv_bulk_kernel<L, BULK_D, BULK_CAP, BULK_WPC>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BULK_SMEM);
+        auto k = bulk_kernel_for<L>(h->spmv_depth);
+        const size_t smem = bulk_smem(h->spmv_depth);
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, BULK_WPC * 32, BULK_SMEM);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, BULK_WPC * 32, smem);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
         int64_t want = (h->num_tiles + BULK_WPC - 1) / BULK_WPC;
@@ -326,6 +339,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "lanes" && (value == 0 || value == 1 || value == 2 || value == 4 || value == 8 || value == 16 || value == 32))
         h->lanes_opt = (int)value;
     else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
+    else if (k == "spmv_depth" && value >= 2 && value <= 4) h->spmv_depth = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -336,6 +350,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     if (k == "lanes") *value = h->lanes;
     else if (k == "spmv_bulk") *value = h->bulk ? 1 : 0;
     else if (k == "spmv_grid") *value = h->spmv_grid;
+    else if (k == "spmv_depth") *value = h->spmv_depth;
     else if (k == "gram_grid") *value = h->gram_grid;
     else if (k == "update_grid") *value = h->update_grid;
     else if (k == "max_row_len") *value = h->max_row_len;
