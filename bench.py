@@ -116,6 +116,25 @@ def dist_env():
     return world, rank, local
 
 
+def dist_ops(world: int, backend: str, device):
+    """(reduce_max, barrier) of the job: identities at world 1, else torch.distributed over `backend`
+    ("nccl" on the GPUs; "gloo" in the CPU test of this host logic).  Used only for timing, never on the data path."""
+    if world == 1:
+        return (lambda v: v), (lambda: None)
+    import torch
+    import torch.distributed as dist
+    if not dist.is_initialized():
+        kw = {"device_id": device} if backend == "nccl" else {}
+        dist.init_process_group(backend, **kw)
+
+    def reduce_max(v):
+        t = torch.tensor([v], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    return reduce_max, dist.barrier
+
+
 def aggregate_replicas(elapsed_ms: float, k_steps: int, world: int, reduce_max) -> dict:
     """Job-level numbers of N independent replicas: time = max over ranks, units = all ranks' outer iterations."""
     t = reduce_max(elapsed_ms)
@@ -160,18 +179,7 @@ def run_ours(args):
     world, rank, local = dist_env()
     assert torch.cuda.is_available(), "bench.py needs a GPU: the hot path has no CPU fallback"
     torch.cuda.set_device(local)
-    reduce_max, barrier = (lambda v: v), (lambda: None)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-        def reduce_max(v):
-            t = torch.tensor([v], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-
-        def barrier():
-            dist.barrier()
+    reduce_max, barrier = dist_ops(world, "nccl", torch.device("cuda", local))
 
     N, s0 = args.grid, args.s
     t0 = time.time()

@@ -87,6 +87,11 @@ __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
+// software prefetch of the cache line holding *p into L2 (no register, no scoreboard entry)
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 // streaming (read-once) 128-bit and 64-bit global loads
 __device__ __forceinline__ double2 ldg_stream2(const double* p) {
     double2 v;

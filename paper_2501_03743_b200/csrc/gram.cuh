@@ -44,7 +44,7 @@ __device__ __forceinline__ int gram_entry(int q, int a, bool& valid) {
 template <int S>
 __global__ void __launch_bounds__(GramCfg<S>::NW * 32)
 gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ AR, const double* __restrict__ AP,
-            const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve) {
+            const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve, int pf) {
     using Cfg = GramCfg<S>;
     constexpr int G = Cfg::G, NSL = Cfg::NSL, RG = Cfg::RG, NW = Cfg::NW, NACC = Cfg::NACC, NE = Cfg::NE;
     if (st->status != SCG_RUNNING) return;
@@ -67,6 +67,20 @@ gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ 
     const int64_t stride = (int64_t)gridDim.x * RG * 32;
     for (int64_t row = ((int64_t)blockIdx.x * RG + rg) * 32 + lane; row < n; row += stride) {
         double Rv[S], ARv[G], APv[G], Rsel[G];
+        if (pf > 0) {  // pull the rows this thread reads `pf` iterations from now into L2 (hides the DRAM latency)
+            const int64_t prow = row + pf * stride;
+            if (prow < n) {
+                if (q == 0) {
+#pragma unroll
+                    for (int j = 0; j < S; j++) prefetch_l2(R + (int64_t)j * n + prow);
+                    prefetch_l2(r + prow);
+                }
+#pragma unroll
+                for (int g = 0; g < G; g++)
+                    if ((G * NSL == S) || (c0 + g < S)) prefetch_l2(AR + (int64_t)(c0 + g) * n + prow);
+                prefetch_l2(AP + prow * S + c0);
+            }
+        }
 #pragma unroll
         for (int j = 0; j < S; j++) Rv[j] = R[(int64_t)j * n + row];
 #pragma unroll

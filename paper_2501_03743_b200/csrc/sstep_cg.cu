@@ -30,7 +30,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, prefetch = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -172,7 +172,7 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
         h->gram_grid = (int)(want < cap ? want : cap);
         return cudaSuccess;
     }
-    gram_kernel<S><<<h->gram_grid, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve);
+    gram_kernel<S><<<h->gram_grid, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve, h->prefetch);
     return cudaGetLastError();
 }
 
@@ -189,7 +189,7 @@ cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, co
         h->update_grid = (int)(want < cap ? want : cap);
         return cudaSuccess;
     }
-    update_kernel<S><<<h->update_grid, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
+    update_kernel<S><<<h->update_grid, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out, h->prefetch);
     return cudaGetLastError();
 }
 
@@ -340,6 +340,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
         h->lanes_opt = (int)value;
     else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
     else if (k == "spmv_depth" && value >= 2 && value <= 4) h->spmv_depth = (int)value;
+    else if (k == "prefetch" && value >= 0 && value <= 16) h->prefetch = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }

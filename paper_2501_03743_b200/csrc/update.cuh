@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(256, 2)
 update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
-              ScgState* __restrict__ st, double* __restrict__ rho_out) {
+              ScgState* __restrict__ st, double* __restrict__ rho_out, int pf) {
     if (st->status != SCG_RUNNING) return;
     __shared__ double sbeta[S * S];
     __shared__ double salpha[S];
@@ -68,6 +68,24 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
     double rho = 0.0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        if (pf > 0) {  // pull the rows this thread reads `pf` iterations from now into L2
+            const int64_t prow = row + pf * stride;
+            if (prow < n) {
+#pragma unroll
+                for (int j = 0; j < S; j++) {
+                    prefetch_l2(R + (int64_t)j * n + prow);
+                    prefetch_l2(AR + (int64_t)j * n + prow);
+                }
+#pragma unroll
+                for (int l = 0; l < S; l += 16) {  // one prefetch per 128-byte line of the interleaved rows
+                    prefetch_l2(P + prow * S + l);
+                    prefetch_l2(AP + prow * S + l);
+                }
+                prefetch_l2(x + prow);
+                prefetch_l2(r + prow);
+                prefetch_l2(dinv + prow);
+            }
+        }
         const double x0 = x[row], r0 = r[row], di = dinv[row];
         const double xi = update_half<S>(n, row, R, P, sbeta, salpha, x0, 1.0);     // P <- R + P beta ; x += P alpha
         const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
