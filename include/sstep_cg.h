@@ -90,6 +90,8 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *   "spmv_variant" 0 auto (default) | 1 force the generic vector-per-row kernel | 2 force the bulk-staged kernel
  *   "lanes"        0 auto | 1,2,4,8,16,32 lanes per row
  *   "spmv_depth"   2 (default) | 3 | 4 slots of the bulk-staged SpMV's per-warp shared-memory ring
+ *   "block_variant" 0 auto (default: Gram/update through the TMA tile pipeline for s >= 5, register kernels below)
+ *                  | 1 force the register kernels | 2 force the tile pipeline
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);

@@ -22,10 +22,9 @@ struct GramCfg {
     static constexpr int NE = 2 * S * S + S;                // Gram entries: M | C | m
 };
 
-// entry index of accumulator a of slice q
-template <int S>
+// entry index (in M | C | m) of accumulator a of slice q, for slices of G columns
+template <int S, int G>
 __device__ __forceinline__ int gram_entry(int q, int a, bool& valid) {
-    constexpr int G = GramCfg<S>::G;
     if (a < S * G) {  // accM[i][g]
         const int i = a / G, col = q * G + a % G;
         valid = col < S;
@@ -41,89 +40,28 @@ __device__ __forceinline__ int gram_entry(int q, int a, bool& valid) {
     return 2 * S * S + col;
 }
 
-template <int S>
-__global__ void __launch_bounds__(GramCfg<S>::NW * 32)
-gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ AR, const double* __restrict__ AP,
-            const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve, int pf) {
-    using Cfg = GramCfg<S>;
-    constexpr int G = Cfg::G, NSL = Cfg::NSL, RG = Cfg::RG, NW = Cfg::NW, NACC = Cfg::NACC, NE = Cfg::NE;
-    if (st->status != SCG_RUNNING) return;
-    __shared__ double red[NW][NACC];
+// ---- everything after the in-warp reduction.  red[g2 * NSL + q][a] holds, for NRED row groups g2 and NSL slices q,
+// the partial sums of the CTA (accumulator order: accM[i][g] at i*G+g, accC[g][i] at S*G+g*S+i, accm[g] at 2*S*G+g).
+// Sums the row groups, writes the per-block partials, takes a ticket; the last block sums all partials in a fixed
+// order (bitwise reproducible) and one warp runs the s x s solves.  Every thread of the CTA must call (barriers).
+template <int S, int G, int NSL, int NRED>
+__device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * S * G + G], double* __restrict__ partials,
+                                                        ScgState* __restrict__ st, int do_solve) {
+    constexpr int NACC = 2 * S * G + G, NE = 2 * S * S + S;
     __shared__ double fin[NE];
     __shared__ SmallSolveSmem ssm;
     __shared__ bool is_last;
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int q = warp % NSL;   // slice
-    const int rg = warp / NSL;  // row group
-    double accM[S][G], accC[G][S], accm[G];
-#pragma unroll
-    for (int g = 0; g < G; g++) {
-        accm[g] = 0.0;
-#pragma unroll
-        for (int i = 0; i < S; i++) { accM[i][g] = 0.0; accC[g][i] = 0.0; }
-    }
-    const int c0 = q * G;
-    const int64_t stride = (int64_t)gridDim.x * RG * 32;
-    for (int64_t row = ((int64_t)blockIdx.x * RG + rg) * 32 + lane; row < n; row += stride) {
-        double Rv[S], ARv[G], APv[G], Rsel[G];
-        if (pf > 0) {  // pull the rows this thread reads `pf` iterations from now into L2 (hides the DRAM latency)
-            const int64_t prow = row + pf * stride;
-            if (prow < n) {
-                if (q == 0) {
-#pragma unroll
-                    for (int j = 0; j < S; j++) prefetch_l2(R + (int64_t)j * n + prow);
-                    prefetch_l2(r + prow);
-                }
-#pragma unroll
-                for (int g = 0; g < G; g++)
-                    if ((G * NSL == S) || (c0 + g < S)) prefetch_l2(AR + (int64_t)(c0 + g) * n + prow);
-                prefetch_l2(AP + prow * S + c0);
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < S; j++) Rv[j] = R[(int64_t)j * n + row];
-#pragma unroll
-        for (int g = 0; g < G; g++) {
-            const bool ok = (G * NSL == S) || (c0 + g < S);
-            ARv[g] = ok ? AR[(int64_t)(c0 + g) * n + row] : 0.0;
-            APv[g] = ok ? AP[row * S + c0 + g] : 0.0;
-            Rsel[g] = ok ? R[(int64_t)(c0 + g) * n + row] : 0.0;  // R_{c0+g} again (L1 hit): keeps Rv[] statically indexed
-        }
-        const double rv = r[row];
-#pragma unroll
-        for (int g = 0; g < G; g++) {
-#pragma unroll
-            for (int i = 0; i < S; i++) {
-                accM[i][g] = fma(Rv[i], ARv[g], accM[i][g]);
-                accC[g][i] = fma(APv[g], Rv[i], accC[g][i]);
-            }
-            accm[g] = fma(Rsel[g], rv, accm[g]);
-        }
-    }
-    // ---- block reduction: shuffle tree inside the warp, then across the RG row groups of a slice ----
-#pragma unroll
-    for (int g = 0; g < G; g++) {
-#pragma unroll
-        for (int i = 0; i < S; i++) {
-            const double a = warp_sum(accM[i][g]);
-            const double b = warp_sum(accC[g][i]);
-            if (lane == 0) { red[warp][i * G + g] = a; red[warp][S * G + g * S + i] = b; }
-        }
-        const double c = warp_sum(accm[g]);
-        if (lane == 0) red[warp][2 * S * G + g] = c;
-    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
     __syncthreads();
     for (int e = threadIdx.x; e < NSL * NACC; e += blockDim.x) {
         const int qs = e / NACC, a = e % NACC;
         double v = 0.0;
 #pragma unroll
-        for (int g2 = 0; g2 < RG; g2++) v += red[g2 * NSL + qs][a];
+        for (int g2 = 0; g2 < NRED; g2++) v += red[g2 * NSL + qs][a];
         bool valid;
-        const int ge = gram_entry<S>(qs, a, valid);
+        const int ge = gram_entry<S, G>(qs, a, valid);
         if (valid) partials[(int64_t)ge * gridDim.x + blockIdx.x] = v;
     }
-    // ---- single-kernel cross-block finish: ticket, last block sums the partials in a fixed order ----
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -133,7 +71,7 @@ gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ 
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    for (int e = warp; e < NE; e += NW) {
+    for (int e = warp; e < NE; e += nwarps) {
         double v = 0.0;
         for (int b = lane; b < (int)gridDim.x; b += 32) v += __ldcg(&partials[(int64_t)e * gridDim.x + b]);
         v = warp_sum(v);
@@ -149,6 +87,66 @@ gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ 
         }
         if (lane == 0) st->ticket_gram = 0;  // re-arm for the next graph replay
     }
+}
+
+template <int S>
+__global__ void __launch_bounds__(GramCfg<S>::NW * 32, 2)
+gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ AR, const double* __restrict__ AP,
+            const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve) {
+    using Cfg = GramCfg<S>;
+    constexpr int G = Cfg::G, NSL = Cfg::NSL, RG = Cfg::RG;
+    if (st->status != SCG_RUNNING) return;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int q = warp % NSL;   // slice
+    const int rg = warp / NSL;  // row group
+    double accM[S][G], accC[G][S], accm[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+        accm[g] = 0.0;
+#pragma unroll
+        for (int i = 0; i < S; i++) { accM[i][g] = 0.0; accC[g][i] = 0.0; }
+    }
+    const int c0 = q * G;
+    const int64_t stride = (int64_t)gridDim.x * RG * 32;
+    for (int64_t row = ((int64_t)blockIdx.x * RG + rg) * 32 + lane; row < n; row += stride) {
+        // all loads of the row first, as one batch (asm volatile keeps them ahead of the FMAs: memory-level parallelism
+        // is what this kernel lives on).  With one slice (S <= 4) nothing is re-read, so the loads bypass L1.
+        double Rv[S], ARv[G], APv[G], Rsel[G];
+#pragma unroll
+        for (int j = 0; j < S; j++) Rv[j] = (NSL == 1) ? ldg_stream(R + (int64_t)j * n + row) : ldg_nc(R + (int64_t)j * n + row);
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+            const bool ok = (G * NSL == S) || (c0 + g < S);
+            ARv[g] = ok ? ldg_stream(AR + (int64_t)(c0 + g) * n + row) : 0.0;
+            APv[g] = ok ? ldg_stream(AP + row * S + c0 + g) : 0.0;
+            if constexpr (NSL == 1) Rsel[g] = Rv[g];
+            else Rsel[g] = ok ? ldg_nc(R + (int64_t)(c0 + g) * n + row) : 0.0;  // R_{c0+g} again (L1 hit): keeps Rv[] statically indexed
+        }
+        const double rv = ldg_stream(r + row);
+#pragma unroll
+        for (int g = 0; g < G; g++) {
+#pragma unroll
+            for (int i = 0; i < S; i++) {
+                accM[i][g] = fma(Rv[i], ARv[g], accM[i][g]);
+                accC[g][i] = fma(APv[g], Rv[i], accC[g][i]);
+            }
+            accm[g] = fma(Rsel[g], rv, accm[g]);
+        }
+    }
+    // ---- block reduction: shuffle tree inside the warp (slice q = warp % NSL, row group rg = warp / NSL) ----
+    __shared__ double red[Cfg::NW][Cfg::NACC];
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+#pragma unroll
+        for (int i = 0; i < S; i++) {
+            const double a = warp_sum(accM[i][g]);
+            const double b = warp_sum(accC[g][i]);
+            if (lane == 0) { red[warp][i * G + g] = a; red[warp][S * G + g * S + i] = b; }
+        }
+        const double c = warp_sum(accm[g]);
+        if (lane == 0) red[warp][2 * S * G + g] = c;
+    }
+    gram_cross_block_finish<S, G, NSL, RG>(red, partials, st, do_solve);
 }
 
 // stand-alone a3 for the test hook: same device function, operands in global memory

@@ -9,8 +9,10 @@
 
 #include "common.cuh"
 #include "gram.cuh"
+#include "gram_tma.cuh"
 #include "spmv.cuh"
 #include "update.cuh"
+#include "update_tma.cuh"
 
 namespace {
 
@@ -30,7 +32,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, prefetch = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -51,6 +53,8 @@ struct sstep_cg {
     int lanes = 1;
     bool bulk = false;
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0;
+    bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
+    int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int64_t num_tiles = 0;
     int max_row_len = 0;
     cudaGraph_t graph = nullptr;
@@ -158,10 +162,13 @@ cudaError_t config_spmv(sstep_cg* h) {
     }
 }
 
+inline bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
+
 template <int S>
 cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R, const double* AR, const double* AP,
                    const double* r, ScgState* st, int do_solve) {
     using Cfg = GramCfg<S>;
+    using TC = GramTmaCfg<S>;
     if (configure) {
         int occ = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_kernel<S>, Cfg::NW * 32, 0);
@@ -169,16 +176,33 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
         if (occ < 1) occ = 1;
         int64_t want = (h->n + Cfg::RG * 32 - 1) / (Cfg::RG * 32);
         int64_t cap = (int64_t)occ * h->num_sms;
-        h->gram_grid = (int)(want < cap ? want : cap);
+        h->gram_grid_reg = h->gram_grid = (int)(want < cap ? want : cap);
+        if (h->staged) {
+            e = cudaFuncSetAttribute(gram_tma_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC::SMEM);
+            if (e != cudaSuccess) return e;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_tma_kernel<S>, TC::THREADS, TC::SMEM);
+            if (e != cudaSuccess) return e;
+            if (occ < 1) occ = 1;
+            want = (h->n + TC::T - 1) / TC::T;
+            cap = (int64_t)occ * h->num_sms;
+            h->gram_grid = (int)(want < cap ? want : cap);
+            if (h->gram_grid < h->gram_grid_reg) h->gram_grid_reg = h->gram_grid;  // partials are sized by gram_grid
+        }
         return cudaSuccess;
     }
-    gram_kernel<S><<<h->gram_grid, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve, h->prefetch);
+    if (h->staged && aligned16(R) && aligned16(AR) && aligned16(AP) && aligned16(r)) {
+        gram_tma_kernel<S><<<h->gram_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve,
+                                                                        (h->n + TC::T - 1) / TC::T);
+    } else {
+        gram_kernel<S><<<h->gram_grid_reg, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve);
+    }
     return cudaGetLastError();
 }
 
 template <int S>
 cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
                      double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
+    using TC = UpdateTmaCfg<S>;
     if (configure) {
         int occ = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_kernel<S>, 256, 0);
@@ -186,10 +210,26 @@ cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, co
         if (occ < 1) occ = 1;
         int64_t want = (h->n + 255) / 256;
         int64_t cap = (int64_t)occ * h->num_sms;
-        h->update_grid = (int)(want < cap ? want : cap);
+        h->update_grid_reg = h->update_grid = (int)(want < cap ? want : cap);
+        if (h->staged) {
+            e = cudaFuncSetAttribute(update_tma_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC::SMEM);
+            if (e != cudaSuccess) return e;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_tma_kernel<S>, TC::THREADS, TC::SMEM);
+            if (e != cudaSuccess) return e;
+            if (occ < 1) occ = 1;
+            want = (h->n + TC::T - 1) / TC::T;
+            cap = (int64_t)occ * h->num_sms;
+            h->update_grid = (int)(want < cap ? want : cap);
+            if (h->update_grid < h->update_grid_reg) h->update_grid_reg = h->update_grid;
+        }
         return cudaSuccess;
     }
-    update_kernel<S><<<h->update_grid, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out, h->prefetch);
+    if (h->staged && aligned16(R) && aligned16(AR) && aligned16(P) && aligned16(AP) && aligned16(x) && aligned16(r)) {
+        update_tma_kernel<S><<<h->update_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
+                                                                            h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
+    } else {
+        update_kernel<S><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
+    }
     return cudaGetLastError();
 }
 
@@ -340,7 +380,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
         h->lanes_opt = (int)value;
     else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
     else if (k == "spmv_depth" && value >= 2 && value <= 4) h->spmv_depth = (int)value;
-    else if (k == "prefetch" && value >= 0 && value <= 16) h->prefetch = (int)value;
+    else if (k == "block_variant" && value >= 0 && value <= 2) h->block_variant = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -352,6 +392,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "spmv_bulk") *value = h->bulk ? 1 : 0;
     else if (k == "spmv_grid") *value = h->spmv_grid;
     else if (k == "spmv_depth") *value = h->spmv_depth;
+    else if (k == "block_staged") *value = h->staged ? 1 : 0;
     else if (k == "gram_grid") *value = h->gram_grid;
     else if (k == "update_grid") *value = h->update_grid;
     else if (k == "max_row_len") *value = h->max_row_len;
@@ -422,6 +463,8 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         return fail(h, SSTEP_CG_ERR_ARG, "setup: bulk SpMV forced but a tile exceeds the staging capacity or arrays are not 16 B aligned");
     }
     h->lanes = L;
+    // Gram / update: register kernels for s <= 4 (they reach the copy peak), TMA tile pipeline above
+    h->staged = (h->block_variant == 2) || (h->block_variant == 0 && s >= 5);
     CK(config_spmv(h));
     CK(launch_gram(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, 0));
     CK(launch_update(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr));

@@ -10,6 +10,46 @@
 #pragma once
 #include "common.cuh"
 
+// V_new(row, :) = Xcol(row, :) + V(row, :) beta ; acc += sign * V_new(row, :) alpha.  Per output column the sum runs
+// over l in ascending order and acc over j in ascending order (the order of update_half); beta is read from shared
+// memory as 128-bit pairs (two output columns per load).
+template <int S>
+__device__ __forceinline__ double update_row(const double (&v)[S], double (&out)[S], const double* sbeta,
+                                             const double* salpha, double acc, double sign) {
+    if constexpr (S % 2 == 0) {
+#pragma unroll
+        for (int l = 0; l < S; l++) {
+            const double2* b2 = reinterpret_cast<const double2*>(sbeta + l * S);
+#pragma unroll
+            for (int j = 0; j < S / 2; j++) {
+                const double2 b = b2[j];
+                out[2 * j] = fma(v[l], b.x, out[2 * j]);
+                out[2 * j + 1] = fma(v[l], b.y, out[2 * j + 1]);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int l = 0; l < S; l++)
+#pragma unroll
+            for (int j = 0; j < S; j++) out[j] = fma(v[l], sbeta[l * S + j], out[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < S; j++) acc = fma(sign * out[j], salpha[j], acc);
+    return acc;
+}
+
+template <int S>
+__device__ __forceinline__ void store_row(double* __restrict__ dst, const double (&out)[S]) {
+    if constexpr (S % 2 == 0) {
+        double2* d2 = reinterpret_cast<double2*>(dst);
+#pragma unroll
+        for (int l = 0; l < S / 2; l++) d2[l] = make_double2(out[2 * l], out[2 * l + 1]);
+    } else {
+#pragma unroll
+        for (int l = 0; l < S; l++) dst[l] = out[l];
+    }
+}
+
 // one half of the update for one row: V <- Xcol + V beta (V = P or AP, interleaved), acc <- acc + sign * (V_new alpha)
 template <int S>
 __device__ __forceinline__ double update_half(int64_t n, int64_t row, const double* __restrict__ Xcm, double* __restrict__ Vil,
@@ -50,57 +90,18 @@ __device__ __forceinline__ double update_half(int64_t n, int64_t row, const doub
     return acc;
 }
 
-template <int S>
-__global__ void __launch_bounds__(256, 2)
-update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
-              double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
-              const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
-              ScgState* __restrict__ st, double* __restrict__ rho_out, int pf) {
-    if (st->status != SCG_RUNNING) return;
-    __shared__ double sbeta[S * S];
-    __shared__ double salpha[S];
-    __shared__ double red[8];
+// ---- ||r||^2 finish shared by the update kernels: block reduce over the first `nw` warps, per-block partial, ticket,
+// fixed-order sum in the last block, then k <- k + 1 and the stop test (Alg. 3 l.31-33).  Every thread of the CTA calls.
+__device__ __forceinline__ void update_block_finish(double rho, int nw, double* __restrict__ partials,
+                                                    ScgState* __restrict__ st, double* __restrict__ rho_out) {
+    __shared__ double red[32];
     __shared__ bool is_last;
-    for (int e = threadIdx.x; e < S * S; e += blockDim.x) sbeta[e] = beta_g[e];
-    if (threadIdx.x < S) salpha[threadIdx.x] = alpha_g[threadIdx.x];
-    __syncthreads();
-
-    double rho = 0.0;
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
-        if (pf > 0) {  // pull the rows this thread reads `pf` iterations from now into L2
-            const int64_t prow = row + pf * stride;
-            if (prow < n) {
-#pragma unroll
-                for (int j = 0; j < S; j++) {
-                    prefetch_l2(R + (int64_t)j * n + prow);
-                    prefetch_l2(AR + (int64_t)j * n + prow);
-                }
-#pragma unroll
-                for (int l = 0; l < S; l += 16) {  // one prefetch per 128-byte line of the interleaved rows
-                    prefetch_l2(P + prow * S + l);
-                    prefetch_l2(AP + prow * S + l);
-                }
-                prefetch_l2(x + prow);
-                prefetch_l2(r + prow);
-                prefetch_l2(dinv + prow);
-            }
-        }
-        const double x0 = x[row], r0 = r[row], di = dinv[row];
-        const double xi = update_half<S>(n, row, R, P, sbeta, salpha, x0, 1.0);     // P <- R + P beta ; x += P alpha
-        const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
-        x[row] = xi;
-        r[row] = ri;
-        R[row] = di * ri;  // R(:,1) of the next outer iteration
-        rho = fma(ri, ri, rho);
-    }
-    // ---- ||r||^2: block reduce, per-block partial, ticket, fixed-order finish in the last block ----
     rho = warp_sum(rho);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = rho;
+    if ((threadIdx.x & 31) == 0 && (int)(threadIdx.x >> 5) < nw) red[threadIdx.x >> 5] = rho;
     __syncthreads();
     if (threadIdx.x == 0) {
         double v = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); w++) v += red[w];
+        for (int w = 0; w < nw; w++) v += red[w];
         partials[blockIdx.x] = v;
         __threadfence();
         const unsigned int t = atomicAdd(&st->ticket_update, 1u);
@@ -122,6 +123,33 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
             st->ticket_update = 0;
         }
     }
+}
+
+template <int S>
+__global__ void __launch_bounds__(256, 2)
+update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
+              double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
+              const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
+              ScgState* __restrict__ st, double* __restrict__ rho_out) {
+    if (st->status != SCG_RUNNING) return;
+    __shared__ __align__(16) double sbeta[S * S];
+    __shared__ double salpha[S];
+    for (int e = threadIdx.x; e < S * S; e += blockDim.x) sbeta[e] = beta_g[e];
+    if (threadIdx.x < S) salpha[threadIdx.x] = alpha_g[threadIdx.x];
+    __syncthreads();
+
+    double rho = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        const double x0 = x[row], r0 = r[row], di = dinv[row];
+        const double xi = update_half<S>(n, row, R, P, sbeta, salpha, x0, 1.0);     // P <- R + P beta ; x += P alpha
+        const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
+        x[row] = xi;
+        r[row] = ri;
+        R[row] = di * ri;  // R(:,1) of the next outer iteration
+        rho = fma(ri, ri, rho);
+    }
+    update_block_finish(rho, (int)(blockDim.x >> 5), partials, st, rho_out);
 }
 
 // ---- start of a solve: r = b - A x0 (Ax0 already in r if have_ax), x = x0, R(:,1) = D^-1 r, rho0 = ||r||^2 ----
