@@ -181,9 +181,10 @@ def run_ours(args):
     torch.cuda.set_device(local)
     reduce_max, barrier = dist_ops(world, "nccl", torch.device("cuda", local))
 
-    N, s0 = args.grid, args.s
+    s0 = args.s
     t0 = time.time()
-    c = gen.make_config(4, N=N)
+    c = gen.make_config(args.config, N=args.grid if args.config == 4 else (args.grid_override or None))
+    N = c["N"]
     t_gen = time.time() - t0
     n, nnz = c["n"], c["nnz"]
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda(local)
@@ -342,6 +343,10 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--s", type=int, default=4, help="block size of the headline value (paper uses s <= 5)")
     ap.add_argument("--grid", type=int, default=320, help="grid edge N of config 4 (N^3 unknowns)")
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6],
+                    help="BASELINE.json config (4 = the headline workload; the others fill BASELINE.md's table; 6 = the "
+                         "paper's own 250^3, b = 1 problem).  The reference arm and the roofline always describe what ran.")
+    ap.add_argument("--grid-override", type=int, default=0, help="grid edge for --config != 4 (0 = the config's own)")
     ap.add_argument("--sweep", type=str, default="1,2,4,8", help="block sizes also reported (config 4's sweep); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -385,8 +390,10 @@ def main():
         "dtype": "f64",
         "data": "synthetic",
         "config": {
-            "workload": f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, b=A x*, x*~U[-1,1] seed 3, "
-                        f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)",
+            "workload": (f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, b=A x*, x*~U[-1,1] seed 3, "
+                         f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)") if args.config == 4 else
+                        (f"config {args.config} ({ctx['c']['name']}): grid {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, x0=0, Jacobi, "
+                         f"s={s}, rtol=0 (fixed iteration count)"),
             "s": s, "grid": N, "restart_every": restart_every_for(s),
             "l2": "inputs larger than L2: one outer iteration streams %.1f GB >> 126 MB" % (mb["total"] / 1e9),
             "parallelism": "replicas only (north_star: one GPU, no sharding)" if world > 1 else "single GPU",
