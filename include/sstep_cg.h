@@ -92,6 +92,11 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *   "spmv_depth"   2 (default) | 3 | 4 slots of the bulk-staged SpMV's per-warp shared-memory ring
  *   "block_variant" 0 auto (default: Gram/update through the TMA tile pipeline for s >= 5, register kernels below)
  *                  | 1 force the register kernels | 2 force the tile pipeline
+ *   "form"         0 (default) Gram form: fused block inner products M, C, m + Cholesky solves (a2, a3)
+ *                  | 1 moment form (paper-literal Alg. 5 + Alg. 6): the 2s moments are accumulated
+ *                    in the SpMV epilogues (mu^0 in the update kernel), a one-block kernel runs the scalar work `SW`;
+ *                    no Gram pass over R, AR, AP, r.  Monomial basis only; less robust (Hankel assumption, division
+ *                    by alpha_prev(s)).
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);
@@ -138,6 +143,13 @@ const char *sstep_cg_last_error(sstep_cg_t *handle);
 int sstep_cg_test_spmv(sstep_cg_t *handle, const double *x, double *y, double *yjac);
 /* a1, Alg. 4: R(:,1) = D^-1 r, then the s fused SpMVs.  R, AR column-major n x s. */
 int sstep_cg_test_mpk(sstep_cg_t *handle, const double *r, double *R_cm, double *AR_cm);
+/* moment form (option form = 1): Alg. 4 as above and the 2s moments vm[k] = mu^k the SpMV epilogues leave
+ * (mu^0 = R_1^T r, mu^{2j-1} = R_j^T AR_j, mu^{2j} = R_{j+1}^T AR_j).  vm: 2s doubles, device. */
+int sstep_cg_test_mpk_moments(sstep_cg_t *handle, const double *r, double *R_cm, double *AR_cm, double *vm);
+/* Alg. 6 `SW`: from the 2s moments vm and (first == 0) the previous alpha, W (passed in alpha / W, overwritten):
+ * beta, alpha, W; first != 0: W = M, beta = 0, alpha = W^-1 vm(1:s).  status_out[0] = 0 or SSTEP_CG_BREAKDOWN. */
+int sstep_cg_test_sw(sstep_cg_t *handle, const double *vm, int first, double *beta, double *alpha, double *W,
+                     int32_t *status_out);
 /* a2: M = R^T AR, C = AP^T R, m = R^T r.  R, AR column-major; AP interleaved; M, C (s*s), m (s) device outputs. */
 int sstep_cg_test_gram(sstep_cg_t *handle, const double *R_cm, const double *AR_cm, const double *AP_il,
                        const double *r, double *M, double *C, double *m);

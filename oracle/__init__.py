@@ -102,6 +102,15 @@ def cvm(R, AR, r):
     return vm
 
 
+def cvm_fused(R, AR, r):
+    """The 2s moments where the MPK produces them: mu^0 = R_1.r, mu^{2j-1} = R_j.AR_j, mu^{2j} = R_{j+1}.AR_j."""
+    R = _f64(R); AR = _f64(AR); r = _f64(r)
+    s, n = R.shape
+    vm = np.empty(2 * s)
+    lib().orc_cvm_fused(C.c_int64(n), C.c_int(s), _p(R), _p(AR), _p(r), _p(vm))
+    return vm
+
+
 def chol(W):
     W = _f64(W); s = W.shape[0]
     L = np.empty((s, s))
@@ -176,7 +185,8 @@ def pfcg(rowptr, colidx, vals, b, x0=None, rtol=1e-8, maxit=2000, history=False,
 
 def sstep(rowptr, colidx, vals, b, s, x0=None, rtol=1e-8, maxit=2000, form="gram", basis=0,
           history=False, xhist_cap=0):
-    """Alg. 3 PCGs; form 'gram' (O2) or 'moment' (O3, Alg. 5 + Alg. 6); iters = outer iterations."""
-    f = {"gram": 0, "moment": 1}[form]
+    """Alg. 3 PCGs; form 'gram' (O2), 'moment' (O3, Alg. 5 + Alg. 6) or 'moment_fused' (O3 with the moments taken
+    in the MPK, cvm_fused); iters = outer iterations."""
+    f = {"gram": 0, "moment": 1, "moment_fused": 2}[form]
     return _solver_common(lib().orc_sstep, rowptr, colidx, vals, b, x0, rtol, maxit,
                           (C.c_int(s), C.c_int(f), C.c_int(basis)), history, xhist_cap)

@@ -135,6 +135,19 @@ void orc_cvm(i64 n, int s, const double *R, const double *AR, const double *r, d
     }
 }
 
+/* The same 2s moments taken where the matrix-powers kernel produces them (Eq. 4,
+ * mu^k = r^T B^{-1} (A B^{-1})^k r):
+ *   mu^0 = R_1^T r,  mu^{2j-1} = R_j^T AR_j,  mu^{2j} = R_{j+1}^T AR_j  (j = 1..s; mu^{2s} is not needed).
+ * In exact arithmetic vm[k] = mu^k equals orc_cvm's vm (A symmetric); in fp64 the two differ by rounding. */
+void orc_cvm_fused(i64 n, int s, const double *R, const double *AR, const double *r, double *vm)
+{
+    vm[0] = (double)ldot(n, R, r);
+    for (int j = 1; j <= s; j++) {
+        vm[2 * j - 1] = (double)ldot(n, R + (i64)(j - 1) * n, AR + (i64)(j - 1) * n);
+        if (j < s) vm[2 * j] = (double)ldot(n, R + (i64)j * n, AR + (i64)(j - 1) * n);
+    }
+}
+
 /* ---------------------------------------------------------------- small solves
  * "solve s+1 spd systems of dimension s".  Method (reading A10):
  * Cholesky W = L L^T reading only the lower triangle of W, then forward and
@@ -415,7 +428,8 @@ int orc_sstep(i64 n, const i32 *rp, const i32 *ci, const double *v, const double
             st = orc_small_solve(s, k == 0, M, C, m, W, beta, alpha, Wn);
             memcpy(W, Wn, sizeof(double) * s * s);
         } else {
-            orc_cvm(n, s, R, AR, r, vm);                               /* l.6 / l.24 */
+            if (form == 2) orc_cvm_fused(n, s, R, AR, r, vm);          /* moments from the MPK epilogues */
+            else orc_cvm(n, s, R, AR, r, vm);                          /* l.6 / l.24 */
             if (k == 0) {                                              /* l.7-14 */
                 for (int i = 1; i <= s; i++)
                     for (int j = 1; j <= s; j++) W[(i - 1) * s + (j - 1)] = vm[i + j - 1];

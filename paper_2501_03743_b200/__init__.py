@@ -23,7 +23,8 @@ STATUS_NAMES = {0: "converged", 1: "maxit", 2: "breakdown"}
 EXPORTED_SYMBOLS = [
     "sstep_cg_create", "sstep_cg_setup", "sstep_cg_set_option", "sstep_cg_get_info", "sstep_cg_solve",
     "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_profile_outer", "sstep_cg_solve_host", "sstep_cg_destroy",
-    "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_gram",
+    "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
+    "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update",
 ]
 
@@ -72,6 +73,8 @@ def load_library(build: bool = True):
     lib.sstep_cg_last_error.restype = C.c_char_p
     lib.sstep_cg_test_spmv.argtypes = [vp, vp, vp, vp]
     lib.sstep_cg_test_mpk.argtypes = [vp, vp, vp, vp]
+    lib.sstep_cg_test_mpk_moments.argtypes = [vp, vp, vp, vp, vp]
+    lib.sstep_cg_test_sw.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     lib.sstep_cg_test_gram.argtypes = [vp] + [vp] * 7
     lib.sstep_cg_test_small_solve.argtypes = [vp] + [vp] * 8
     lib.sstep_cg_test_update.argtypes = [vp] + [vp] * 9
@@ -236,6 +239,31 @@ class SStepCG:
         AR = torch.empty_like(R)
         self._check(self._lib.sstep_cg_test_mpk(self._h, self._ptr(r), self._ptr(R), self._ptr(AR)), "sstep_cg_test_mpk")
         return R, AR
+
+    def test_mpk_moments(self, r):
+        """Moment form: R, AR as in test_mpk plus the 2s moments vm[k] = mu^k left by the SpMV epilogues."""
+        torch = _torch()
+        r = self._dev(r, torch.float64, "r", self.n)
+        R = torch.empty((self.s, self.n), dtype=torch.float64, device=r.device)
+        AR = torch.empty_like(R)
+        vm = torch.empty(2 * self.s, dtype=torch.float64, device=r.device)
+        self._check(self._lib.sstep_cg_test_mpk_moments(self._h, self._ptr(r), self._ptr(R), self._ptr(AR), self._ptr(vm)),
+                    "sstep_cg_test_mpk_moments")
+        return R, AR, vm
+
+    def test_sw(self, vm, alpha_prev=None, W_prev=None):
+        """Alg. 6: (status, beta, alpha, W); alpha_prev / W_prev None = first outer iteration."""
+        torch = _torch()
+        s = self.s
+        vm = self._dev(vm, torch.float64, "vm", 2 * s)
+        first = alpha_prev is None
+        alpha = torch.zeros(s, dtype=torch.float64, device=vm.device) if first else self._dev(alpha_prev, torch.float64, "alpha", s).clone()
+        W = torch.zeros((s, s), dtype=torch.float64, device=vm.device) if first else self._dev(W_prev, torch.float64, "W", s * s).clone()
+        beta = torch.zeros((s, s), dtype=torch.float64, device=vm.device)
+        st = torch.zeros(1, dtype=torch.int32, device=vm.device)
+        self._check(self._lib.sstep_cg_test_sw(self._h, self._ptr(vm), 1 if first else 0, self._ptr(beta), self._ptr(alpha),
+                                               self._ptr(W), self._ptr(st)), "sstep_cg_test_sw")
+        return int(st.item()), beta, alpha, W
 
     def test_gram(self, R, AR, AP, r):
         torch = _torch()

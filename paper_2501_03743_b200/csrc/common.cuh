@@ -22,6 +22,9 @@ struct ScgState {
     double M[SCG_SMAX * SCG_SMAX];
     double C[SCG_SMAX * SCG_SMAX];
     double m[SCG_SMAX];
+    // ---- moment form (option "form" = 1): mu^0 = R_1^T r from the update / init kernel, the 2s moments of the last MPK
+    double mu0;
+    double vm[2 * SCG_SMAX];
     // ---- cross-block finish tickets (reset by the last block, so graphs can be replayed) ----
     unsigned int ticket_gram;
     unsigned int ticket_update;

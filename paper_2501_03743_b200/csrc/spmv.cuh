@@ -25,13 +25,32 @@ __device__ __forceinline__ void spmv_epilogue(int64_t row, double acc, const dou
     }
 }
 
+// Moment form: per-block partial sums of  mu_a = sum_rows x_i (A x)_i  and  mu_b = sum_rows (D^-1 A x)_i (A x)_i
+// (for SpMV j of the MPK these are mu^{2j-1} = R_j^T AR_j and mu^{2j} = R_{j+1}^T AR_j; Eq. 4).
+// Every thread of the CTA calls; one double per block and moment, summed later in fixed block order by sw_kernel.
+__device__ __forceinline__ void spmv_moment_finish(double ma, double mb, double* __restrict__ mom_a, double* __restrict__ mom_b) {
+    __shared__ double red[2][32];
+    ma = warp_sum(ma);
+    mb = warp_sum(mb);
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = ma; red[1][threadIdx.x >> 5] = mb; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { a += red[0][w]; b += red[1][w]; }
+        mom_a[blockIdx.x] = a;
+        if (mom_b) mom_b[blockIdx.x] = b;
+    }
+}
+
 template <int L>
 __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci,
                                                        const double* __restrict__ va, const double* __restrict__ dinv,
                                                        const double* __restrict__ x, double* __restrict__ y,
                                                        double* __restrict__ yjac, const double* __restrict__ xprev, int mode,
-                                                       const ScgState* __restrict__ st) {
+                                                       const ScgState* __restrict__ st, double* __restrict__ mom_a,
+                                                       double* __restrict__ mom_b) {
     if (st && st->status != SCG_RUNNING) return;
+    double ma = 0.0, mb = 0.0;  // moment partials x^T (A x) and (D^-1 A x)^T (A x), see spmv_moment_finish
     const int g = threadIdx.x % L;
     const int64_t rows_per_pass = (int64_t)gridDim.x * (blockDim.x / L);
     // the loop runs on the warp's first row so that all 32 lanes reach the shuffles the same number of times
@@ -43,10 +62,19 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
         int lo = 0, hi = 0;
         if (live) { lo = rp[row]; hi = rp[row + 1]; }
         double acc = 0.0;
+        // plain loop on purpose: batching the index/value loads by hand (and streaming hints on them) measured
+        // 20-90 % slower -- consecutive iterations re-use the sectors of colidx/vals through L1
         for (int k = lo + g; k < hi; k += L) acc = fma(va[k], x[ci[k]], acc);
         acc = group_sum<L>(acc);
-        if (live && g == 0) spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
+        if (live && g == 0) {
+            spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
+            if (mom_a) {
+                ma = fma(x[row], acc, ma);
+                if (yjac) mb = fma(dinv[row] * acc, acc, mb);
+            }
+        }
     }
+    if (mom_a) spmv_moment_finish(ma, mb, mom_a, mom_b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -63,7 +91,7 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
 template <int U>
 struct SpmvFrag {
     double v[U], xv[U];
-    double diag, rem, xrow, xprev;
+    double diag, xdiag, rem, xrow, xprev;
 };
 
 template <int L, int D, int CAP, int WPC>
@@ -71,7 +99,8 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
                                                              const int* __restrict__ ci, const double* __restrict__ va,
                                                              const double* __restrict__ x, double* __restrict__ y,
                                                              double* __restrict__ yjac, const double* __restrict__ xprev,
-                                                             int mode, const ScgState* __restrict__ st, int64_t num_tiles) {
+                                                             int mode, const ScgState* __restrict__ st, int64_t num_tiles,
+                                                             double* __restrict__ mom_a, double* __restrict__ mom_b) {
     if (st && st->status != SCG_RUNNING) return;
     constexpr int RPT = 32 / L;
     constexpr int U = 8;  // entries per lane held in registers (rows up to 8 L entries need no remainder loop)
@@ -90,8 +119,8 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
     const uint64_t policy = l2_policy_evict_first();
     const int64_t GW = (int64_t)gridDim.x * WPC;
     const int64_t gw = (int64_t)blockIdx.x * WPC + warp;
-    if (gw >= num_tiles) return;
-    const int64_t my_tiles = (num_tiles - gw + GW - 1) / GW;
+    const int64_t my_tiles = (gw < num_tiles) ? (num_tiles - gw + GW - 1) / GW : 0;
+    double ma = 0.0, mb = 0.0;  // moment partials (moment form only)
     const int g = lane % L;
     const bool jac = yjac != nullptr;
 
@@ -155,6 +184,10 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
         }
 #pragma unroll
         for (int u = 0; u < U; u++) f.xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
+        f.xdiag = 0.0;
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (c[u] == row) f.xdiag = f.xv[u];
         f.xrow = 0.0;
         f.xprev = 0.0;
         if (jac && mode != 0 && row < n) {
@@ -165,8 +198,9 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
         for (int k = lo + g + U * L; k < hi; k += L) {  // long rows only
             const int cc = sc[k];
             const double vv = sv[k];
-            if (cc == row) f.diag = vv;
-            rem = fma(vv, x[cc], rem);
+            const double xx = x[cc];
+            if (cc == row) { f.diag = vv; f.xdiag = xx; }
+            rem = fma(vv, xx, rem);
         }
         f.rem = rem;
         __syncwarp();  // every lane has read the slot: it may be refilled
@@ -180,10 +214,14 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
         acc = group_sum<L>(acc);
         double d = f.diag;
         if (L > 1 && jac) d = group_sum<L>(d);  // exactly one lane of the group holds a_ii, the others 0
+        double xd = f.xdiag;
+        if (L > 1 && mom_a) xd = group_sum<L>(xd);
         if (g == 0 && row < n) {
             y[row] = acc;
+            if (mom_a) ma = fma(xd, acc, ma);
             if (jac) {
                 double z = __drcp_rn(d) * acc;  // = (1 / a_ii) * acc, the same two roundings as a dinv array
+                if (mom_a) mb = fma(z, acc, mb);
                 if (mode == 1) z = z - f.xrow;
                 else if (mode == 2) z = 2.0 * (z - f.xrow) - f.xprev;
                 yjac[row] = z;
@@ -222,6 +260,7 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
             finish(i, cur);
         }
     }
+    if (mom_a) spmv_moment_finish(ma, mb, mom_a, mom_b);
 }
 
 // max nnz over tiles of `rpt` rows (setup-time check for the bulk variant)

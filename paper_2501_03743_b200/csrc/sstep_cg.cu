@@ -10,6 +10,7 @@
 #include "common.cuh"
 #include "gram.cuh"
 #include "gram_tma.cuh"
+#include "moment.cuh"
 #include "spmv.cuh"
 #include "update.cuh"
 #include "update_tma.cuh"
@@ -32,7 +33,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -43,6 +44,7 @@ struct sstep_cg {
     // owned device memory
     double *dinv = nullptr, *R = nullptr, *AR = nullptr, *P = nullptr, *AP = nullptr, *x = nullptr, *r = nullptr;
     double* partials = nullptr;
+    double* mom = nullptr;        // moment form: [2s][spmv_grid] per-block partials of mu^1 .. mu^{2s-1}
     ScgState* st = nullptr;       // production state
     ScgState* st_test = nullptr;  // state used by the test hooks
     int* iscratch = nullptr;      // [err, max_len, max_tile]
@@ -86,7 +88,7 @@ int fail(sstep_cg* h, int code, const std::string& msg) {
 
 // ---------------------------------------------------------------- kernel dispatch
 using bulk_fn_t = void (*)(int64_t, int64_t, const int*, const int*, const double*, const double*, double*, double*,
-                           const double*, int, const ScgState*, int64_t);
+                           const double*, int, const ScgState*, int64_t, double*, double*);
 
 template <int L>
 bulk_fn_t bulk_kernel_for(int depth) {
@@ -99,26 +101,26 @@ bulk_fn_t bulk_kernel_for(int depth) {
 
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
-                          int mode, const ScgState* st) {
+                          int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if (h->bulk) {
         bulk_kernel_for<L>(h->spmv_depth)<<<h->spmv_grid, BULK_WPC * 32, bulk_smem(h->spmv_depth), sm>>>(
-            h->n, h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->num_tiles);
+            h->n, h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->num_tiles, mom_a, mom_b);
     } else {
-        spmv_vec_kernel<L><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st);
+        spmv_vec_kernel<L><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
     }
     return cudaGetLastError();
 }
 
 cudaError_t launch_spmv(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
-                        int mode, const ScgState* st) {
+                        int mode, const ScgState* st, double* mom_a = nullptr, double* mom_b = nullptr) {
     h->launches++;
     switch (h->lanes) {
-        case 1: return launch_spmv_L<1>(h, sm, x, y, yjac, xprev, mode, st);
-        case 2: return launch_spmv_L<2>(h, sm, x, y, yjac, xprev, mode, st);
-        case 4: return launch_spmv_L<4>(h, sm, x, y, yjac, xprev, mode, st);
-        case 8: return launch_spmv_L<8>(h, sm, x, y, yjac, xprev, mode, st);
-        case 16: return launch_spmv_L<16>(h, sm, x, y, yjac, xprev, mode, st);
-        default: return launch_spmv_L<32>(h, sm, x, y, yjac, xprev, mode, st);
+        case 1: return launch_spmv_L<1>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        case 2: return launch_spmv_L<2>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        case 4: return launch_spmv_L<4>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        case 8: return launch_spmv_L<8>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        case 16: return launch_spmv_L<16>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        default: return launch_spmv_L<32>(h, sm, x, y, yjac, xprev, mode, st, mom_a, mom_b);
     }
 }
 
@@ -276,17 +278,27 @@ cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, cons
             mode = (j == 0) ? 1 : 2;
             if (j > 0) xprev = R + (int64_t)(j - 1) * n;
         }
-        cudaError_t e = launch_spmv(h, sm, R + (int64_t)j * n, AR + (int64_t)j * n, yjac, xprev, mode, st);
+        // moment form: SpMV j (1-based) also leaves the per-block partials of mu^{2j-1} = R_j^T AR_j and mu^{2j} = R_{j+1}^T AR_j
+        double* mom_a = h->form ? h->mom + (int64_t)(2 * j + 1) * h->spmv_grid : nullptr;
+        double* mom_b = (h->form && j + 1 < h->s) ? h->mom + (int64_t)(2 * j + 2) * h->spmv_grid : nullptr;
+        cudaError_t e = launch_spmv(h, sm, R + (int64_t)j * n, AR + (int64_t)j * n, yjac, xprev, mode, st, mom_a, mom_b);
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+// moment form, after the MPK: fixed-order sum of the moment partials + Alg. 6 in one warp (replaces the Gram kernel)
+cudaError_t launch_sw(sstep_cg* h, cudaStream_t sm, ScgState* st, int do_solve) {
+    h->launches++;
+    sw_kernel<<<1, 256, 0, sm>>>(h->s, h->spmv_grid, h->mom, st, do_solve);
+    return cudaGetLastError();
 }
 
 // one outer iteration on the production buffers (Alg. 3 l.5-21)
 cudaError_t launch_outer(sstep_cg* h, cudaStream_t sm) {
     cudaError_t e = launch_mpk(h, sm, h->R, h->AR, h->st);
     if (e != cudaSuccess) return e;
-    e = launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1);
+    e = h->form ? launch_sw(h, sm, h->st, 1) : launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1);
     if (e != cudaSuccess) return e;
     return launch_update(h, sm, false, h->R, h->AR, h->P, h->AP, h->x, h->r, h->st->beta, h->st->alpha, h->st, nullptr);
 }
@@ -296,7 +308,7 @@ void free_problem(sstep_cg* h) {
     if (h->graph) cudaGraphDestroy(h->graph);
     h->gexec = nullptr;
     h->graph = nullptr;
-    double** bufs[] = {&h->dinv, &h->R, &h->AR, &h->P, &h->AP, &h->x, &h->r, &h->partials};
+    double** bufs[] = {&h->dinv, &h->R, &h->AR, &h->P, &h->AP, &h->x, &h->r, &h->partials, &h->mom};
     for (double** b : bufs) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -381,6 +393,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
     else if (k == "spmv_depth" && value >= 2 && value <= 4) h->spmv_depth = (int)value;
     else if (k == "block_variant" && value >= 0 && value <= 2) h->block_variant = (int)value;
+    else if (k == "form" && (value == 0 || value == 1)) h->form = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -393,6 +406,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "spmv_grid") *value = h->spmv_grid;
     else if (k == "spmv_depth") *value = h->spmv_depth;
     else if (k == "block_staged") *value = h->staged ? 1 : 0;
+    else if (k == "form") *value = h->form;
     else if (k == "gram_grid") *value = h->gram_grid;
     else if (k == "update_grid") *value = h->update_grid;
     else if (k == "max_row_len") *value = h->max_row_len;
@@ -410,6 +424,8 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     if (n <= 0 || nnz <= 0 || nnz >= (int64_t(1) << 31) || n >= (int64_t(1) << 31) || !rowptr || !colidx || !vals || s < 1 ||
         s > SSTEP_CG_SMAX)
         return fail(h, SSTEP_CG_ERR_ARG, "setup: need n > 0, 0 < nnz < 2^31, non-null CSR arrays, 1 <= s <= 16");
+    if (h->form == 1 && h->basis != SSTEP_CG_BASIS_MONOMIAL)
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: the moment form (Alg. 5 + Alg. 6) assumes the monomial basis");
     CK(cudaSetDevice(h->device));
     CK(cudaStreamSynchronize(h->stream));
     free_problem(h);
@@ -440,7 +456,10 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     if (h->lanes_opt) L = h->lanes_opt;
     h->bulk = false;
     const bool aligned = (((uintptr_t)colidx | (uintptr_t)vals) & 15) == 0;
-    if (h->spmv_variant != 1 && aligned) {
+    // auto: the bulk-staged kernel for thread-per-row matrices (mean row <= 8 entries, e.g. 7-point stencils), where it
+    // reaches ~95 % of the copy peak; with several lanes per row the generic kernel is faster (27-point 160^3: 269 vs
+    // 356 us).  Forced (spmv_variant = 2): any L whose tiles fit.
+    if ((h->spmv_variant == 2 || (h->spmv_variant == 0 && L == 1)) && aligned) {
         for (int Lb = L; Lb <= 32; Lb *= 2) {
             const int rpt = 32 / Lb;
             const int64_t tiles = (n + rpt - 1) / rpt;
@@ -455,7 +474,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
                 h->num_tiles = tiles;
                 break;
             }
-            if (h->lanes_opt) break;
+            if (h->lanes_opt || h->spmv_variant == 0) break;
         }
     }
     if (h->spmv_variant == 2 && !h->bulk) {
@@ -482,9 +501,11 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     CK(cudaMalloc(&h->x, sizeof(double) * n));
     CK(cudaMalloc(&h->r, sizeof(double) * n));
     size_t np = (size_t)h->gram_grid * (2 * s * s + s);
-    if (np < (size_t)h->update_grid) np = h->update_grid;
-    if (np < (size_t)h->init_grid) np = h->init_grid;
+    if (np < 2 * (size_t)h->update_grid) np = 2 * (size_t)h->update_grid;
+    if (np < 2 * (size_t)h->init_grid) np = 2 * (size_t)h->init_grid;
     CK(cudaMalloc(&h->partials, sizeof(double) * np));
+    CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
+    CK(cudaMemsetAsync(h->mom, 0, sizeof(double) * 2 * s * (size_t)h->spmv_grid, sm));
     CK(cudaMemsetAsync(h->R, 0, blk, sm));
     CK(cudaMemsetAsync(h->AR, 0, blk, sm));
     CK(cudaMemsetAsync(h->P, 0, blk, sm));
@@ -569,11 +590,13 @@ int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
                     if (j > 0) xprev = h->R + (int64_t)(j - 1) * n;
                 }
                 CK(cudaEventRecord(evs[e++], sm));
-                CK(launch_spmv(h, sm, h->R + (int64_t)j * n, h->AR + (int64_t)j * n, yjac, xprev, mode, h->st));
+                double* mom_a = h->form ? h->mom + (int64_t)(2 * j + 1) * h->spmv_grid : nullptr;
+                double* mom_b = (h->form && j + 1 < h->s) ? h->mom + (int64_t)(2 * j + 2) * h->spmv_grid : nullptr;
+                CK(launch_spmv(h, sm, h->R + (int64_t)j * n, h->AR + (int64_t)j * n, yjac, xprev, mode, h->st, mom_a, mom_b));
                 CK(cudaEventRecord(evs[e++], sm));
             }
             CK(cudaEventRecord(evs[e++], sm));
-            CK(launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1));
+            CK(h->form ? launch_sw(h, sm, h->st, 1) : launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1));
             CK(cudaEventRecord(evs[e++], sm));
             CK(cudaEventRecord(evs[e++], sm));
             CK(launch_update(h, sm, false, h->R, h->AR, h->P, h->AP, h->x, h->r, h->st->beta, h->st->alpha, h->st, nullptr));
@@ -716,6 +739,30 @@ int sstep_cg_test_mpk(sstep_cg_t* h, const double* r, double* R, double* AR) {
     init_kernel<<<h->init_grid, 256, 0, h->stream>>>(h->n, r, nullptr, 0, h->x, h->r, R, h->dinv, h->partials, h->st_test, h->s, 0.0);
     CK(cudaGetLastError());
     CK(launch_mpk(h, h->stream, R, AR, h->st_test));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_mpk_moments(sstep_cg_t* h, const double* r, double* R, double* AR, double* vm) {
+    if (!h || !r || !R || !AR || !vm) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    if (!h->form) return fail(h, SSTEP_CG_ERR_STATE, "test_mpk_moments: set option form = 1 before setup");
+    init_kernel<<<h->init_grid, 256, 0, h->stream>>>(h->n, r, nullptr, 0, h->x, h->r, R, h->dinv, h->partials, h->st_test, h->s, 0.0);
+    CK(cudaGetLastError());
+    CK(launch_mpk(h, h->stream, R, AR, h->st_test));
+    CK(launch_sw(h, h->stream, h->st_test, 0));
+    CK(cudaMemcpyAsync(vm, h->st_test->vm, sizeof(double) * 2 * h->s, cudaMemcpyDeviceToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_sw(sstep_cg_t* h, const double* vm, int first, double* beta, double* alpha, double* W, int32_t* status_out) {
+    if (!h || !vm || !beta || !alpha || !W || !status_out) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    sw_test_kernel<<<1, 32, 0, h->stream>>>(h->s, first, vm, beta, alpha, W, status_out);
+    CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
     return 0;
 }

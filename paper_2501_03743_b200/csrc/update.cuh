@@ -90,19 +90,22 @@ __device__ __forceinline__ double update_half(int64_t n, int64_t row, const doub
     return acc;
 }
 
-// ---- ||r||^2 finish shared by the update kernels: block reduce over the first `nw` warps, per-block partial, ticket,
-// fixed-order sum in the last block, then k <- k + 1 and the stop test (Alg. 3 l.31-33).  Every thread of the CTA calls.
-__device__ __forceinline__ void update_block_finish(double rho, int nw, double* __restrict__ partials,
+// ---- ||r||^2 (and mu^0 = R_1^T r of the moment form) finish shared by the update kernels: block reduce over the first
+// `nw` warps, per-block partials, ticket, fixed-order sum in the last block, then k <- k + 1 and the stop test
+// (Alg. 3 l.31-33).  partials: [2][gridDim.x].  Every thread of the CTA calls.
+__device__ __forceinline__ void update_block_finish(double rho, double mu0, int nw, double* __restrict__ partials,
                                                     ScgState* __restrict__ st, double* __restrict__ rho_out) {
-    __shared__ double red[32];
+    __shared__ double red[2][32];
     __shared__ bool is_last;
     rho = warp_sum(rho);
-    if ((threadIdx.x & 31) == 0 && (int)(threadIdx.x >> 5) < nw) red[threadIdx.x >> 5] = rho;
+    mu0 = warp_sum(mu0);
+    if ((threadIdx.x & 31) == 0 && (int)(threadIdx.x >> 5) < nw) { red[0][threadIdx.x >> 5] = rho; red[1][threadIdx.x >> 5] = mu0; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double v = 0.0;
-        for (int w = 0; w < nw; w++) v += red[w];
+        double v = 0.0, w = 0.0;
+        for (int i = 0; i < nw; i++) { v += red[0][i]; w += red[1][i]; }
         partials[blockIdx.x] = v;
+        partials[gridDim.x + blockIdx.x] = w;
         __threadfence();
         const unsigned int t = atomicAdd(&st->ticket_update, 1u);
         is_last = (t == gridDim.x - 1);
@@ -111,11 +114,13 @@ __device__ __forceinline__ void update_block_finish(double rho, int nw, double* 
     if (!is_last) return;
     if (threadIdx.x < 32) {
         __threadfence();
-        double v = 0.0;
-        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) v += __ldcg(&partials[b]);
+        double v = 0.0, w = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) { v += __ldcg(&partials[b]); w += __ldcg(&partials[gridDim.x + b]); }
         v = warp_sum(v);
+        w = warp_sum(w);
         if (threadIdx.x == 0) {
             st->rho = v;
+            st->mu0 = w;
             st->k = st->k + 1;
             if (rho_out) rho_out[0] = v;
             if (!isfinite(v)) st->status = 2;
@@ -138,7 +143,7 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
     if (threadIdx.x < S) salpha[threadIdx.x] = alpha_g[threadIdx.x];
     __syncthreads();
 
-    double rho = 0.0;
+    double rho = 0.0, mu0 = 0.0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
         const double x0 = x[row], r0 = r[row], di = dinv[row];
@@ -146,10 +151,12 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
         const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
         x[row] = xi;
         r[row] = ri;
-        R[row] = di * ri;  // R(:,1) of the next outer iteration
+        const double r1 = di * ri;
+        R[row] = r1;  // R(:,1) of the next outer iteration
         rho = fma(ri, ri, rho);
+        mu0 = fma(r1, ri, mu0);
     }
-    update_block_finish(rho, (int)(blockDim.x >> 5), partials, st, rho_out);
+    update_block_finish(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
 }
 
 // ---- start of a solve: r = b - A x0 (Ax0 already in r if have_ax), x = x0, R(:,1) = D^-1 r, rho0 = ||r||^2 ----
@@ -157,24 +164,28 @@ __global__ void __launch_bounds__(256)
 init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ x0, int have_ax, double* __restrict__ x,
             double* __restrict__ r, double* __restrict__ R, const double* __restrict__ dinv, double* __restrict__ partials,
             ScgState* __restrict__ st, int s, double rtol) {
-    __shared__ double red[8];
+    __shared__ double red[2][8];
     __shared__ bool is_last;
-    double rho = 0.0;
+    double rho = 0.0, mu0 = 0.0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
         const double ri = have_ax ? b[row] - r[row] : b[row];
+        const double r1 = dinv[row] * ri;
         x[row] = x0 ? x0[row] : 0.0;
         r[row] = ri;
-        R[row] = dinv[row] * ri;
+        R[row] = r1;
         rho = fma(ri, ri, rho);
+        mu0 = fma(r1, ri, mu0);
     }
     rho = warp_sum(rho);
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = rho;
+    mu0 = warp_sum(mu0);
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = rho; red[1][threadIdx.x >> 5] = mu0; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double v = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); w++) v += red[w];
+        double v = 0.0, u = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { v += red[0][w]; u += red[1][w]; }
         partials[blockIdx.x] = v;
+        partials[gridDim.x + blockIdx.x] = u;
         __threadfence();
         const unsigned int t = atomicAdd(&st->ticket_init, 1u);
         is_last = (t == gridDim.x - 1);
@@ -183,9 +194,10 @@ init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ 
     if (!is_last) return;
     if (threadIdx.x < 32) {
         __threadfence();
-        double v = 0.0;
-        for (int bk = threadIdx.x; bk < (int)gridDim.x; bk += 32) v += __ldcg(&partials[bk]);
+        double v = 0.0, u = 0.0;
+        for (int bk = threadIdx.x; bk < (int)gridDim.x; bk += 32) { v += __ldcg(&partials[bk]); u += __ldcg(&partials[gridDim.x + bk]); }
         v = warp_sum(v);
+        u = warp_sum(u);
         for (int e = threadIdx.x; e < s * s; e += 32) {
             st->W[e] = (e / s == e % s) ? 1.0 : 0.0;  // W_prev = I with C = 0 gives beta = 0, W = M at k = 0
             st->beta[e] = 0.0;
@@ -193,6 +205,7 @@ init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ 
         if (threadIdx.x == 0) {
             st->rho = v;
             st->rho0 = v;
+            st->mu0 = u;
             st->rtol = rtol;
             st->k = 0;
             st->status = (v == 0.0) ? 0 : (isfinite(v) ? SCG_RUNNING : 2);

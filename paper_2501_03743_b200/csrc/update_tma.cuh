@@ -63,7 +63,7 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
     }
     __syncthreads();
 
-    double rho = 0.0;
+    double rho = 0.0, mu0 = 0.0;
     const int64_t my_tiles = ((int64_t)blockIdx.x < num_tiles) ? (num_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
 
     if (warp >= NCW) {
@@ -148,8 +148,10 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
             if (live) {
                 x[row] = xi;
                 r[row] = ri;
-                R[row] = di * ri;  // R(:,1) of the next outer iteration
+                const double r1 = di * ri;
+                R[row] = r1;  // R(:,1) of the next outer iteration
                 rho = fma(ri, ri, rho);
+                mu0 = fma(r1, ri, mu0);
             }
             if (lane == 0) {
                 if constexpr (S % 2 == 0) bulk_wait_read();  // the stores have read the slot: it may be refilled
@@ -159,5 +161,5 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
         }
         if (lane == 0) bulk_wait_all();
     }
-    update_block_finish(rho, NCW, partials, st, rho_out);
+    update_block_finish(rho, mu0, NCW, partials, st, rho_out);
 }

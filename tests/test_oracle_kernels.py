@@ -161,6 +161,28 @@ def hilbert_inverse(n):
     return H
 
 
+@pytest.mark.parametrize("s", [1, 2, 4, 8])
+def test_cvm_fused_closed_form_and_symmetry(oracle_mod, s):
+    """The moments taken in the MPK epilogues (cvm_fused): (a) closed form for an eigenvector input,
+    mu^k = lam^k ||r||^2 / d^(k+1); (b) for a general r they equal Alg. 5's moments (cvm) because A is symmetric
+    (Eq. 4) -- two different sets of inner products, so a wrong index or column fails here."""
+    N = 9
+    rp, ci, v = gen.poisson7(N)
+    vec, lam = poisson7_eigvec(N, 1, 2, 3)
+    dinv = oracle_mod.dinv(rp, ci, v)
+    R, AR = oracle_mod.mpk(rp, ci, v, dinv, vec, s)
+    vm = oracle_mod.cvm_fused(R, AR, vec)
+    expect = np.array([lam ** k * (vec @ vec) / 6.0 ** (k + 1) for k in range(2 * s)])
+    assert np.allclose(vm, expect, rtol=1e-12, atol=0)
+    c = gen.make_config(5, N=7)                        # variable diagonal, permuted: D^-1 does not commute with A
+    rp, ci, v = c["rowptr"], c["colidx"], c["vals"]
+    dinv = oracle_mod.dinv(rp, ci, v)
+    r = np.random.default_rng(9).uniform(-1, 1, c["n"])
+    R, AR = oracle_mod.mpk(rp, ci, v, dinv, r, s)
+    a, b = oracle_mod.cvm_fused(R, AR, r), oracle_mod.cvm(R, AR, r)
+    assert np.allclose(a, b, rtol=1e-10, atol=0)
+
+
 @pytest.mark.parametrize("s", [1, 2, 3, 4, 5, 6])
 def test_cholesky_hilbert_closed_form(oracle_mod, s):
     H = 1.0 / (np.arange(1, s + 1)[:, None] + np.arange(1, s + 1)[None, :] - 1.0)

@@ -46,7 +46,7 @@ def test_tiny_spd_converges_to_lu(oracle_mod, name, rp, ci, v, A):
     # s-step: when s does not divide the grade of b the last block [R_1..R_s] is rank deficient and W is
     # singular (exact breakdown, see test_rank_deficient_last_block); take s | 64 there.
     for s in ((1, 2, 3, 4) if name == "rand48" else (1, 2, 4)):
-        for form in ("gram", "moment"):
+        for form in ("gram", "moment", "moment_fused"):
             runs.append((f"s{s}{form}", oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-9, maxit=-(-n // s) + 2, form=form), s))
     for tag, res, s in runs:
         assert res["status"] == 0, (tag, res["relres"])
@@ -89,7 +89,7 @@ def test_sstep_iterates_equal_cg_every_s_steps(oracle_mod, c, s):
     ref2 = oracle_mod.pfcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=0.0, maxit=nouter * s, xhist_cap=nouter * s)
     scale = np.linalg.norm(ref["xhist"][-1])
     assert np.abs(ref["xhist"] - ref2["xhist"]).max() <= 1e-13 * scale          # Alg. 1 == Alg. 2
-    for form in ("gram", "moment"):
+    for form in ("gram", "moment", "moment_fused"):
         res = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=0.0, maxit=nouter, form=form,
                                xhist_cap=nouter)
         assert res["status"] == 1 and res["iters"] == nouter
