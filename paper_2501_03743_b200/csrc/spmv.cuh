@@ -42,7 +42,7 @@ __device__ __forceinline__ void spmv_moment_finish(double ma, double mb, double*
     }
 }
 
-template <int L>
+template <int L, bool MOM>
 __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci,
                                                        const double* __restrict__ va, const double* __restrict__ dinv,
                                                        const double* __restrict__ x, double* __restrict__ y,
@@ -68,13 +68,13 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
         acc = group_sum<L>(acc);
         if (live && g == 0) {
             spmv_epilogue(row, acc, dinv, x, xprev, mode, y, yjac);
-            if (mom_a) {
+            if (MOM) {
                 ma = fma(x[row], acc, ma);
                 if (yjac) mb = fma(dinv[row] * acc, acc, mb);
             }
         }
     }
-    if (mom_a) spmv_moment_finish(ma, mb, mom_a, mom_b);
+    if (MOM) spmv_moment_finish(ma, mb, mom_a, mom_b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -91,15 +91,15 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
 template <int U>
 struct SpmvFrag {
     double v[U], xv[U];
-    double diag, xdiag, rem, xrow, xprev;
+    double diag, rem, xrow, xprev;
 };
 
-template <int L, int D, int CAP, int WPC>
-__global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp,
+template <int L, int D, int CAP, int WPC, bool MOM>
+__global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int n, int nnz, const int* __restrict__ rp,
                                                              const int* __restrict__ ci, const double* __restrict__ va,
                                                              const double* __restrict__ x, double* __restrict__ y,
                                                              double* __restrict__ yjac, const double* __restrict__ xprev,
-                                                             int mode, const ScgState* __restrict__ st, int64_t num_tiles,
+                                                             int mode, const ScgState* __restrict__ st, int num_tiles,
                                                              double* __restrict__ mom_a, double* __restrict__ mom_b) {
     if (st && st->status != SCG_RUNNING) return;
     constexpr int RPT = 32 / L;
@@ -117,19 +117,21 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
     }
     __syncwarp();
     const uint64_t policy = l2_policy_evict_first();
-    const int64_t GW = (int64_t)gridDim.x * WPC;
-    const int64_t gw = (int64_t)blockIdx.x * WPC + warp;
-    const int64_t my_tiles = (gw < num_tiles) ? (num_tiles - gw + GW - 1) / GW : 0;
+    // 32-bit row / tile arithmetic (setup guarantees n + 64 < 2^31): keeps the kernel inside its 80-register budget
+    const int GW = (int)gridDim.x * WPC;
+    const int gw = (int)blockIdx.x * WPC + warp;
+    if (!MOM && gw >= num_tiles) return;  // (the moment form ends in a block-wide reduction: every warp stays)
+    const int my_tiles = (gw < num_tiles) ? (num_tiles - gw + GW - 1) / GW : 0;
     double ma = 0.0, mb = 0.0;  // moment partials (moment form only)
     const int g = lane % L;
     const bool jac = yjac != nullptr;
 
     // issue the copies of this warp's i-th tile into slot i % D; nz0/nz1 = its nnz range (valid in lane 0)
-    auto issue = [&](int64_t i, int nz0, int nz1) {
+    auto issue = [&](int i, int nz0, int nz1) {
         const int sl = (int)(i % D);
         const int a0 = nz0 & ~3;
         int bulk_end = (nz1 + 3) & ~3;
-        const int lim = (int)(nnz & ~(int64_t)3);
+        const int lim = nnz & ~3;
         if (bulk_end > lim) bulk_end = lim;
         if (bulk_end < a0) bulk_end = a0;
         const int cnt = bulk_end - a0;
@@ -154,20 +156,20 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
             dc[e - b_a0] = ci[e];
         }
     };
-    auto tile_bounds = [&](int64_t i, int& nz0, int& nz1) {  // lane 0 only
-        const int64_t t = gw + i * GW;
-        const int64_t row0 = t * RPT;
-        int64_t row1 = row0 + RPT;
+    auto tile_bounds = [&](int i, int& nz0, int& nz1) {  // lane 0 only
+        const int t = gw + i * GW;
+        const int row0 = t * RPT;
+        int row1 = row0 + RPT;
         if (row1 > n) row1 = n;
         nz0 = rp[row0];
         nz1 = rp[row1];
     };
-    auto row_of = [&](int64_t i) { return (gw + i * GW) * RPT + lane / L; };
+    auto row_of = [&](int i) { return (gw + i * GW) * RPT + lane / L; };
 
     // slot i % D -> registers (waits for the copy; reads this lane's entries; issues the x gather)
-    auto load_frag = [&](int64_t i, int lo, int hi, SpmvFrag<U>& f) {
+    auto load_frag = [&](int i, int lo, int hi, SpmvFrag<U>& f) {
         const int sl = (int)(i % D);
-        const int64_t row = row_of(i);
+        const int row = row_of(i);
         const int a0 = __shfl_sync(0xffffffffu, lo, 0) & ~3;
         mbar_wait(&bars[sl], (uint32_t)((i / D) & 1));
         const double* sv = svals + sl * CAP - a0;
@@ -184,13 +186,9 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
         }
 #pragma unroll
         for (int u = 0; u < U; u++) f.xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
-        f.xdiag = 0.0;
-#pragma unroll
-        for (int u = 0; u < U; u++)
-            if (c[u] == row) f.xdiag = f.xv[u];
         f.xrow = 0.0;
         f.xprev = 0.0;
-        if (jac && mode != 0 && row < n) {
+        if ((MOM || (jac && mode != 0)) && row < n) {  // x_row: Chebyshev epilogue, and the moment x^T (A x)
             f.xrow = x[row];
             if (mode == 2) f.xprev = xprev[row];
         }
@@ -199,14 +197,14 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
             const int cc = sc[k];
             const double vv = sv[k];
             const double xx = x[cc];
-            if (cc == row) { f.diag = vv; f.xdiag = xx; }
+            if (cc == row) f.diag = vv;
             rem = fma(vv, xx, rem);
         }
         f.rem = rem;
         __syncwarp();  // every lane has read the slot: it may be refilled
     };
-    auto finish = [&](int64_t i, const SpmvFrag<U>& f) {
-        const int64_t row = row_of(i);
+    auto finish = [&](int i, const SpmvFrag<U>& f) {
+        const int row = row_of(i);
         double acc = 0.0;
 #pragma unroll
         for (int u = 0; u < U; u++) acc = fma(f.v[u], f.xv[u], acc);
@@ -214,31 +212,29 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
         acc = group_sum<L>(acc);
         double d = f.diag;
         if (L > 1 && jac) d = group_sum<L>(d);  // exactly one lane of the group holds a_ii, the others 0
-        double xd = f.xdiag;
-        if (L > 1 && mom_a) xd = group_sum<L>(xd);
         if (g == 0 && row < n) {
             y[row] = acc;
-            if (mom_a) ma = fma(xd, acc, ma);
+            if (MOM) ma = fma(f.xrow, acc, ma);
             if (jac) {
                 double z = __drcp_rn(d) * acc;  // = (1 / a_ii) * acc, the same two roundings as a dinv array
-                if (mom_a) mb = fma(z, acc, mb);
+                if (MOM) mb = fma(z, acc, mb);
                 if (mode == 1) z = z - f.xrow;
                 else if (mode == 2) z = 2.0 * (z - f.xrow) - f.xprev;
                 yjac[row] = z;
             }
         }
     };
-    auto row_bounds = [&](int64_t i, int& lo, int& hi) {
+    auto row_bounds = [&](int i, int& lo, int& hi) {
         lo = hi = 0;
         if (i < my_tiles) {
-            const int64_t row = row_of(i);
+            const int row = row_of(i);
             if (row < n) { lo = rp[row]; hi = rp[row + 1]; }
         }
     };
 
     // prologue: fill the ring
     int nb0 = 0, nb1 = 0;  // nnz range of the next tile to issue (lane 0; fetched one step ahead)
-    for (int64_t i = 0; i < D && i < my_tiles; i++) {
+    for (int i = 0; i < D && i < my_tiles; i++) {
         int a = 0, b = 0;
         if (lane == 0) tile_bounds(i, a, b);
         issue(i, a, b);
@@ -249,7 +245,7 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
     {
         SpmvFrag<U> cur;
         row_bounds(0, lo_n, hi_n);
-        for (int64_t i = 0; i < my_tiles; i++) {
+        for (int i = 0; i < my_tiles; i++) {
             const int lo = lo_n, hi = hi_n;
             row_bounds(i + 1, lo_n, hi_n);
             load_frag(i, lo, hi, cur);
@@ -260,7 +256,7 @@ __global__ void __launch_bounds__(WPC * 32, 3) spmv_bulk_kernel(int64_t n, int64
             finish(i, cur);
         }
     }
-    if (mom_a) spmv_moment_finish(ma, mb, mom_a, mom_b);
+    if (MOM) spmv_moment_finish(ma, mb, mom_a, mom_b);
 }
 
 // max nnz over tiles of `rpt` rows (setup-time check for the bulk variant)

@@ -87,26 +87,29 @@ int fail(sstep_cg* h, int code, const std::string& msg) {
     } while (0)
 
 // ---------------------------------------------------------------- kernel dispatch
-using bulk_fn_t = void (*)(int64_t, int64_t, const int*, const int*, const double*, const double*, double*, double*,
-                           const double*, int, const ScgState*, int64_t, double*, double*);
+using bulk_fn_t = void (*)(int, int, const int*, const int*, const double*, const double*, double*, double*,
+                           const double*, int, const ScgState*, int, double*, double*);
 
-template <int L>
-bulk_fn_t bulk_kernel_for(int depth) {
+template <int L, bool MOM>
+bulk_fn_t bulk_kernel_mom(int depth) {
     switch (depth) {
-        case 2: return spmv_bulk_kernel<L, 2, BULK_CAP, BULK_WPC>;
-        case 3: return spmv_bulk_kernel<L, 3, BULK_CAP, BULK_WPC>;
-        default: return spmv_bulk_kernel<L, 4, BULK_CAP, BULK_WPC>;
+        case 2: return spmv_bulk_kernel<L, 2, BULK_CAP, BULK_WPC, MOM>;
+        case 3: return spmv_bulk_kernel<L, 3, BULK_CAP, BULK_WPC, MOM>;
+        default: return spmv_bulk_kernel<L, 4, BULK_CAP, BULK_WPC, MOM>;
     }
 }
+template <int L>
+bulk_fn_t bulk_kernel_for(int depth, bool mom) { return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth); }
 
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if (h->bulk) {
-        bulk_kernel_for<L>(h->spmv_depth)<<<h->spmv_grid, BULK_WPC * 32, bulk_smem(h->spmv_depth), sm>>>(
-            h->n, h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->num_tiles, mom_a, mom_b);
+        bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr)<<<h->spmv_grid, BULK_WPC * 32, bulk_smem(h->spmv_depth), sm>>>(
+            (int)h->n, (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, (int)h->num_tiles, mom_a, mom_b);
     } else {
-        spmv_vec_kernel<L><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        if (mom_a) spmv_vec_kernel<L, true><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        else spmv_vec_kernel<L, false><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
     }
     return cudaGetLastError();
 }
@@ -129,9 +132,12 @@ cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
     if (h->bulk) {
-        auto k = bulk_kernel_for<L>(h->spmv_depth);
+        auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0);
         const size_t smem = bulk_smem(h->spmv_depth);
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        // (the variant without moments is also launched in the moment form: x0 != 0 start-up, test_spmv hook)
+        e = cudaFuncSetAttribute(bulk_kernel_for<L>(h->spmv_depth, false), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, BULK_WPC * 32, smem);
         if (e != cudaSuccess) return e;
@@ -140,7 +146,7 @@ cudaError_t config_spmv_L(sstep_cg* h) {
         int64_t cap = (int64_t)occ * h->num_sms;
         h->spmv_grid = (int)(want < cap ? want : cap);
     } else {
-        auto k = spmv_vec_kernel<L>;
+        auto k = spmv_vec_kernel<L, false>;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, 0);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
@@ -201,22 +207,22 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
     return cudaGetLastError();
 }
 
-template <int S>
-cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
-                     double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
+template <int S, bool MOM>
+cudaError_t update_SM(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
+                      double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
     using TC = UpdateTmaCfg<S>;
     if (configure) {
         int occ = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_kernel<S>, 256, 0);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_kernel<S, MOM>, 256, 0);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
         int64_t want = (h->n + 255) / 256;
         int64_t cap = (int64_t)occ * h->num_sms;
         h->update_grid_reg = h->update_grid = (int)(want < cap ? want : cap);
         if (h->staged) {
-            e = cudaFuncSetAttribute(update_tma_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC::SMEM);
+            e = cudaFuncSetAttribute(update_tma_kernel<S, MOM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC::SMEM);
             if (e != cudaSuccess) return e;
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_tma_kernel<S>, TC::THREADS, TC::SMEM);
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, update_tma_kernel<S, MOM>, TC::THREADS, TC::SMEM);
             if (e != cudaSuccess) return e;
             if (occ < 1) occ = 1;
             want = (h->n + TC::T - 1) / TC::T;
@@ -227,12 +233,20 @@ cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, co
         return cudaSuccess;
     }
     if (h->staged && aligned16(R) && aligned16(AR) && aligned16(P) && aligned16(AP) && aligned16(x) && aligned16(r)) {
-        update_tma_kernel<S><<<h->update_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
-                                                                            h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
+        update_tma_kernel<S, MOM><<<h->update_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
+                                                                                 h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
     } else {
-        update_kernel<S><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
+        update_kernel<S, MOM><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
     }
     return cudaGetLastError();
+}
+
+// the moment form's update also accumulates mu^0 = R_1^T r (compiled in only there)
+template <int S>
+cudaError_t update_S(sstep_cg* h, cudaStream_t sm, bool configure, double* R, const double* AR, double* P, double* AP,
+                     double* x, double* r, const double* beta, const double* alpha, ScgState* st, double* rho_out) {
+    return h->form ? update_SM<S, true>(h, sm, configure, R, AR, P, AP, x, r, beta, alpha, st, rho_out)
+                   : update_SM<S, false>(h, sm, configure, R, AR, P, AP, x, r, beta, alpha, st, rho_out);
 }
 
 #define SCG_DISPATCH_S(fn, ...)                          \
@@ -459,7 +473,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     // auto: the bulk-staged kernel for thread-per-row matrices (mean row <= 8 entries, e.g. 7-point stencils), where it
     // reaches ~95 % of the copy peak; with several lanes per row the generic kernel is faster (27-point 160^3: 269 vs
     // 356 us).  Forced (spmv_variant = 2): any L whose tiles fit.
-    if ((h->spmv_variant == 2 || (h->spmv_variant == 0 && L == 1)) && aligned) {
+    if ((h->spmv_variant == 2 || (h->spmv_variant == 0 && L == 1)) && aligned && n + 64 < (int64_t(1) << 31)) {
         for (int Lb = L; Lb <= 32; Lb *= 2) {
             const int rpt = 32 / Lb;
             const int64_t tiles = (n + rpt - 1) / rpt;

@@ -92,20 +92,24 @@ __device__ __forceinline__ double update_half(int64_t n, int64_t row, const doub
 
 // ---- ||r||^2 (and mu^0 = R_1^T r of the moment form) finish shared by the update kernels: block reduce over the first
 // `nw` warps, per-block partials, ticket, fixed-order sum in the last block, then k <- k + 1 and the stop test
-// (Alg. 3 l.31-33).  partials: [2][gridDim.x].  Every thread of the CTA calls.
+// (Alg. 3 l.31-33).  partials: [2][gridDim.x].  Every thread of the CTA calls.  MOM: only the moment form pays for mu^0.
+template <bool MOM>
 __device__ __forceinline__ void update_block_finish(double rho, double mu0, int nw, double* __restrict__ partials,
                                                     ScgState* __restrict__ st, double* __restrict__ rho_out) {
-    __shared__ double red[2][32];
+    __shared__ double red[MOM ? 2 : 1][32];
     __shared__ bool is_last;
     rho = warp_sum(rho);
-    mu0 = warp_sum(mu0);
-    if ((threadIdx.x & 31) == 0 && (int)(threadIdx.x >> 5) < nw) { red[0][threadIdx.x >> 5] = rho; red[1][threadIdx.x >> 5] = mu0; }
+    if (MOM) mu0 = warp_sum(mu0);
+    if ((threadIdx.x & 31) == 0 && (int)(threadIdx.x >> 5) < nw) {
+        red[0][threadIdx.x >> 5] = rho;
+        if (MOM) red[MOM ? 1 : 0][threadIdx.x >> 5] = mu0;
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
         double v = 0.0, w = 0.0;
-        for (int i = 0; i < nw; i++) { v += red[0][i]; w += red[1][i]; }
+        for (int i = 0; i < nw; i++) { v += red[0][i]; if (MOM) w += red[MOM ? 1 : 0][i]; }
         partials[blockIdx.x] = v;
-        partials[gridDim.x + blockIdx.x] = w;
+        if (MOM) partials[gridDim.x + blockIdx.x] = w;
         __threadfence();
         const unsigned int t = atomicAdd(&st->ticket_update, 1u);
         is_last = (t == gridDim.x - 1);
@@ -115,12 +119,15 @@ __device__ __forceinline__ void update_block_finish(double rho, double mu0, int 
     if (threadIdx.x < 32) {
         __threadfence();
         double v = 0.0, w = 0.0;
-        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) { v += __ldcg(&partials[b]); w += __ldcg(&partials[gridDim.x + b]); }
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) {
+            v += __ldcg(&partials[b]);
+            if (MOM) w += __ldcg(&partials[gridDim.x + b]);
+        }
         v = warp_sum(v);
-        w = warp_sum(w);
+        if (MOM) w = warp_sum(w);
         if (threadIdx.x == 0) {
             st->rho = v;
-            st->mu0 = w;
+            if (MOM) st->mu0 = w;
             st->k = st->k + 1;
             if (rho_out) rho_out[0] = v;
             if (!isfinite(v)) st->status = 2;
@@ -130,8 +137,8 @@ __device__ __forceinline__ void update_block_finish(double rho, double mu0, int 
     }
 }
 
-template <int S>
-__global__ void __launch_bounds__(256, 2)
+template <int S, bool MOM>
+__global__ void __launch_bounds__(256, (S <= 2) ? 4 : 2)
 update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
@@ -154,9 +161,9 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
         const double r1 = di * ri;
         R[row] = r1;  // R(:,1) of the next outer iteration
         rho = fma(ri, ri, rho);
-        mu0 = fma(r1, ri, mu0);
+        if (MOM) mu0 = fma(r1, ri, mu0);  // moment form: mu^0 = R_1^T r
     }
-    update_block_finish(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
+    update_block_finish<MOM>(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
 }
 
 // ---- start of a solve: r = b - A x0 (Ax0 already in r if have_ax), x = x0, R(:,1) = D^-1 r, rho0 = ||r||^2 ----

@@ -38,7 +38,7 @@ __device__ __forceinline__ void load_row(const double* __restrict__ src, double 
     }
 }
 
-template <int S>
+template <int S, bool MOM>
 __global__ void __launch_bounds__(UpdateTmaCfg<S>::THREADS, UpdateTmaCfg<S>::MINB)
 update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
                   double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
@@ -151,7 +151,7 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
                 const double r1 = di * ri;
                 R[row] = r1;  // R(:,1) of the next outer iteration
                 rho = fma(ri, ri, rho);
-                mu0 = fma(r1, ri, mu0);
+                if (MOM) mu0 = fma(r1, ri, mu0);
             }
             if (lane == 0) {
                 if constexpr (S % 2 == 0) bulk_wait_read();  // the stores have read the slot: it may be refilled
@@ -161,5 +161,5 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
         }
         if (lane == 0) bulk_wait_all();
     }
-    update_block_finish(rho, mu0, NCW, partials, st, rho_out);
+    update_block_finish<MOM>(rho, mu0, NCW, partials, st, rho_out);
 }
