@@ -38,6 +38,22 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// Fixed-order sum of p[0 .. cnt) by one warp (cross-block finishes): lane-strided with four independent accumulators
+// so that the L2 loads overlap; the order depends only on cnt, so the result is reproducible run to run.
+__device__ __forceinline__ double warp_sum_array(const double* p, int cnt, int lane) {
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int b = lane;
+    for (; b + 96 < cnt; b += 128) {
+        const double v0 = __ldcg(p + b), v1 = __ldcg(p + b + 32), v2 = __ldcg(p + b + 64), v3 = __ldcg(p + b + 96);
+        a0 += v0; a1 += v1; a2 += v2; a3 += v3;
+    }
+    for (; b < cnt; b += 32) a0 += __ldcg(p + b);
+    double v = (a0 + a1) + (a2 + a3);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 template <int L>
 __device__ __forceinline__ double group_sum(double v) {
 #pragma unroll

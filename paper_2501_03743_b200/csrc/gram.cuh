@@ -71,18 +71,21 @@ __device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * 
     __syncthreads();
     if (!is_last) return;
     __threadfence();
+    __shared__ double sW[S * S], sbeta[S * S], salpha[S];
     for (int e = warp; e < NE; e += nwarps) {
-        double v = 0.0;
-        for (int b = lane; b < (int)gridDim.x; b += 32) v += __ldcg(&partials[(int64_t)e * gridDim.x + b]);
-        v = warp_sum(v);
+        const double v = warp_sum_array(partials + (int64_t)e * gridDim.x, (int)gridDim.x, lane);
         if (lane == 0) fin[e] = v;
     }
+    if (warp == nwarps - 1)
+        for (int e = lane; e < S * S; e += 32) sW[e] = st->W[e];  // W of the previous outer iteration
     __syncthreads();
     if (warp == 0) {
         for (int e = lane; e < S * S; e += 32) { st->M[e] = fin[e]; st->C[e] = fin[S * S + e]; }
         if (lane < S) st->m[lane] = fin[2 * S * S + lane];
-        if (do_solve) {
-            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, st->W, st->beta, st->alpha, st->W, ssm, lane);
+        if (do_solve) {  // all operands in shared memory: the solves are one long dependent chain
+            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, sW, sbeta, salpha, sW, ssm, lane);
+            for (int e = lane; e < S * S; e += 32) { st->W[e] = sW[e]; st->beta[e] = sbeta[e]; }
+            if (lane < S) st->alpha[lane] = salpha[lane];
             if (lane == 0 && rc != 0) st->status = rc;
         }
         if (lane == 0) st->ticket_gram = 0;  // re-arm for the next graph replay

@@ -70,21 +70,22 @@ __global__ void __launch_bounds__(256) sw_kernel(int s, int nblk, const double* 
     if (st->status != SCG_RUNNING) return;
     __shared__ double vm[2 * SCG_SMAX];
     __shared__ SwSmem sm;
-    __shared__ double al[SCG_SMAX];
+    __shared__ double al[SCG_SMAX], sW[SCG_SMAX * SCG_SMAX], sbeta[SCG_SMAX * SCG_SMAX];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    // rows 1 .. 2s-1 of mom, two warps-worth of work per moment would not help: one warp per moment, loads overlapped
     for (int m = 1 + warp; m < 2 * s; m += nw) {
-        double v = 0.0;
-        for (int b = lane; b < nblk; b += 32) v += __ldcg(&mom[(int64_t)m * nblk + b]);
-        v = warp_sum(v);
+        const double v = warp_sum_array(mom + (int64_t)m * nblk, nblk, lane);
         if (lane == 0) vm[m] = v;
     }
     if (threadIdx.x == 0) vm[0] = st->mu0;
     if (threadIdx.x < s) al[threadIdx.x] = st->alpha[threadIdx.x];
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) sW[e] = st->W[e];
     __syncthreads();
     if (warp == 0) {
         for (int e = lane; e < 2 * s; e += 32) st->vm[e] = vm[e];
-        if (do_solve) {
-            const int rc = warp_sw(s, st->k == 0, vm, st->beta, al, st->W, sm, lane);
+        if (do_solve) {  // all operands in shared memory: Alg. 6 is one long dependent chain
+            const int rc = warp_sw(s, st->k == 0, vm, sbeta, al, sW, sm, lane);
+            for (int e = lane; e < s * s; e += 32) { st->W[e] = sW[e]; st->beta[e] = sbeta[e]; }
             if (lane < s) st->alpha[lane] = al[lane];
             if (lane == 0 && rc != 0) st->status = rc;
         }

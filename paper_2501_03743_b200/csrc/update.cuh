@@ -118,13 +118,9 @@ __device__ __forceinline__ void update_block_finish(double rho, double mu0, int 
     if (!is_last) return;
     if (threadIdx.x < 32) {
         __threadfence();
-        double v = 0.0, w = 0.0;
-        for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) {
-            v += __ldcg(&partials[b]);
-            if (MOM) w += __ldcg(&partials[gridDim.x + b]);
-        }
-        v = warp_sum(v);
-        if (MOM) w = warp_sum(w);
+        const double v = warp_sum_array(partials, (int)gridDim.x, (int)threadIdx.x);
+        double w = 0.0;
+        if (MOM) w = warp_sum_array(partials + gridDim.x, (int)gridDim.x, (int)threadIdx.x);
         if (threadIdx.x == 0) {
             st->rho = v;
             if (MOM) st->mu0 = w;
@@ -201,10 +197,8 @@ init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ 
     if (!is_last) return;
     if (threadIdx.x < 32) {
         __threadfence();
-        double v = 0.0, u = 0.0;
-        for (int bk = threadIdx.x; bk < (int)gridDim.x; bk += 32) { v += __ldcg(&partials[bk]); u += __ldcg(&partials[gridDim.x + bk]); }
-        v = warp_sum(v);
-        u = warp_sum(u);
+        const double v = warp_sum_array(partials, (int)gridDim.x, (int)threadIdx.x);
+        const double u = warp_sum_array(partials + gridDim.x, (int)gridDim.x, (int)threadIdx.x);
         for (int e = threadIdx.x; e < s * s; e += 32) {
             st->W[e] = (e / s == e % s) ? 1.0 : 0.0;  // W_prev = I with C = 0 gives beta = 0, W = M at k = 0
             st->beta[e] = 0.0;
