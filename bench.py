@@ -46,12 +46,33 @@ def model_bytes(n: int, nnz: int, s: int, form: int = 0) -> dict:
     return dict(mpk=mpk, gram=gram, update=update, total=mpk + gram + update, spmv_per_launch=mpk / s)
 
 
+def c_default_grid(config: int) -> int:
+    return {1: 32, 2: 128, 3: 160, 4: 320, 5: 256, 6: 250}[config]
+
+
 def measured_peak():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(config: int, s: int, prefix: str = "spmv"):
+    """Per-launch DRAM bytes (read + write) of the kernels whose name starts with `prefix`, from the committed ncu
+    summary profiles/ncu_traffic.csv (launch-weighted mean), or None if that workload was not captured."""
+    try:
+        tot = cnt = 0.0
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            next(f)
+            for ln in f:
+                c, ss, k, w, rd, wr = ln.split(",")[:6]
+                if int(c) == config and int(ss) == s and k.startswith(prefix):
+                    tot += float(w) * (float(rd) + float(wr))
+                    cnt += float(w)
+        return tot / cnt if cnt else None
+    except Exception:
+        return None
 
 
 def restart_every_for(s: int) -> int:
@@ -420,7 +441,8 @@ def main():
                      "frac": mb["spmv_per_launch"] / k_us / 1e3 / ctx["peak"], "peak_source": ctx["peak_src"],
                      "algorithmic_bytes_per_launch": mb["spmv_per_launch"], "avg_launch_us": k_us,
                      "share_of_step": p["kernel_share_of_step"]["spmv"],
-                     "traffic": None},
+                     "traffic": ncu_traffic(args.config, s) if N == c_default_grid(args.config) else None,
+                     "traffic_source": "profiles/ncu_traffic.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)"},
         "kernels": {"us": p["kernel_us"], "gbs": p["kernel_gbs"], "frac_of_measured_peak": p["kernel_frac_of_measured_peak"],
                     "share_of_step": p["kernel_share_of_step"]},
         "sweep": ctx["sweep"],

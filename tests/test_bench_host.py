@@ -81,3 +81,14 @@ def test_reference_arm_runs_on_rank0_only(monkeypatch):
     class A:
         grid, s, steps, warmup, gpus = 320, 4, 1, 1, 2
     assert bench.run_reference(A) is None
+
+
+def test_ncu_traffic_table_is_read():
+    """roofline.traffic comes from the committed ncu summary: SpMV rows of config 4, s = 4, launch-weighted."""
+    sys.path.insert(0, ROOT)
+    import bench
+    t = bench.ncu_traffic(4, 4)
+    n, nnz = 320 ** 3, 7 * 320 ** 3 - 6 * 320 ** 2
+    alg = bench.model_bytes(n, nnz, 4)["spmv_per_launch"]
+    assert t is not None and 0.95 * alg < t < 1.15 * alg          # measured DRAM traffic within 15 % of the algorithmic bytes
+    assert bench.ncu_traffic(4, 3) is None and bench.ncu_traffic(9, 4) is None
