@@ -117,6 +117,31 @@ def test_iterate_trajectory_matches_oracle(oracle_mod, cg_mod, torch_mod):
             assert res["kernel_launches"] == 1 + k * h.get_info("kernels_per_outer")
 
 
+@pytest.mark.parametrize("form", [0, 1])
+def test_s1_pipeline_is_the_papers_fcg_comparator(oracle_mod, cg_mod, torch_mod, form):
+    """At s = 1 the pipeline is Alg. 2 PFCG-NN step by step (u = B^-1 r, w = A u, the three coupled dots
+    alpha = u.r, beta = u.w, gamma = u.s_prev in one reduction, rho = beta - gamma^2/rho_prev, the two axpy pairs;
+    PAPER.md:87-126) -- the paper's baseline "fcg".  Its iterates equal the oracle's Alg. 2 (and Alg. 1) iterates, and a
+    full solve takes the same number of iterations (reading A15)."""
+    c = gen.make_config(4, N=24)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    ref2 = oracle_mod.pfcg(rp, ci, v, b, rtol=0.0, maxit=8, xhist_cap=8)
+    ref1 = oracle_mod.pcg(rp, ci, v, b, rtol=0.0, maxit=8, xhist_cap=8)
+    with cg_mod.SStepCG(0, form=form) as h:
+        h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), 1)
+        bd = dev(torch_mod, b)
+        for k in (1, 2, 5, 8):
+            h.solve_begin(bd, None, 0.0)
+            h.iterate(k)
+            x, res = h.solve_end()
+            assert rel(x.cpu().numpy(), ref2["xhist"][k - 1]) <= 1e-12
+            assert rel(x.cpu().numpy(), ref1["xhist"][k - 1]) <= 1e-12
+        full2 = oracle_mod.pfcg(rp, ci, v, b, rtol=1e-8, maxit=2000)
+        x, res = h.solve(bd, rtol=1e-8, maxit=2000)
+        assert res["status"] == 0 and abs(res["outer_iters"] - full2["iters"]) <= 1
+        assert rel(x.cpu().numpy(), full2["x"]) <= 1e-8
+
+
 def test_graph_and_direct_launch_agree_bitwise(cg_mod, torch_mod):
     c = gen.make_config(1, N=24)
     xs = []
