@@ -167,6 +167,7 @@ def aggregate_replicas(elapsed_ms: float, k_steps: int, world: int, reduce_max) 
 def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
     """CUDA-event time (ms) of exactly k_steps outer iterations (graph replays) on the solver's stream."""
     R = restart_every_for(s)
+    resident = h.get_info("resident") == 1      # whole loop in one cooperative launch: init + 1 launch per restart
     h.solve_begin(b, None, 0.0)
     h.iterate(warmup)
     _, res = h.solve_end(want_x=False)
@@ -181,7 +182,7 @@ def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
         h.solve_begin(b, None, 0.0)
         h.iterate(k)
         done += k
-        launches += 1 + k * (s + 2)
+        launches += 2 if resident else 1 + k * (s + 2)
     ev1.record()
     torch.cuda.synchronize()
     barrier()
@@ -219,7 +220,7 @@ def run_ours(args):
     runs = [(0, s) for s in s_list] + ([(1, s) for s in s_list] if args.moment_form else [])
     moment = {}
     for form, s in runs:
-        with cg.SStepCG(local, form=form) as h:
+        with cg.SStepCG(local, form=form, resident=1) as h:      # graph path: one launch per kernel, per-kernel times
             h.setup(rp, ci, va, s)
             info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid")}
             if s == s0 and form == 0:
@@ -258,7 +259,19 @@ def run_ours(args):
             sweep[str(s)] = entry
             if s == s0:
                 primary = dict(entry, launches=launches, agg=agg, mb=mb)
+    # resident path: what sstep_cg_solve runs by default when every CTA's rows fit shared memory
+    resident = None
+    with cg.SStepCG(local) as h:
+        h.setup(rp, ci, va, s0)
+        if h.get_info("resident") == 1:
+            ms, launches, res = time_outer_iterations(torch, h, b, s0, args.steps, args.warmup, barrier)
+            agg = aggregate_replicas(ms, args.steps, world, reduce_max)
+            resident = dict(s=s0, us_per_outer=1e3 * agg["ms_per_step"], launches=launches, grid=h.get_info("resident_grid"),
+                            rows_per_cta=h.get_info("resident_rows_per_block"), smem_bytes=h.get_info("resident_smem_bytes"),
+                            gdof_iter_per_s=world * n * s0 / (1e3 * agg["ms_per_step"] * 1e-6) / 1e9, relres_at_end=res["relres"],
+                            note="whole loop in one cooperative launch per restart (csrc/resident.cuh); s + 1 grid barriers per outer iteration")
     return dict(world=world, rank=rank, local=local, c=c, n=n, nnz=nnz, N=N, sweep=sweep, moment=moment, primary=primary, clocks=clocks,
+                resident=resident,
                 peak=peak, peak_src=peak_src, t_gen=t_gen, dev=(rp, ci, va, b))
 
 
@@ -446,6 +459,7 @@ def main():
         "kernels": {"us": p["kernel_us"], "gbs": p["kernel_gbs"], "frac_of_measured_peak": p["kernel_frac_of_measured_peak"],
                     "share_of_step": p["kernel_share_of_step"]},
         "sweep": ctx["sweep"],
+        "resident_path": ctx["resident"],  # only for problems that fit shared memory (config 1), else null
         "moment_form": ctx["moment"],     # same solver with Alg. 5 + Alg. 6 (no Gram pass); not the headline
         "clocks": ctx["clocks"],
         "gpu_launches": p["launches"],

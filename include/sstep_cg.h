@@ -97,6 +97,11 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                    in the SpMV epilogues (mu^0 in the update kernel), a one-block kernel runs the scalar work `SW`;
  *                    no Gram pass over R, AR, AP, r.  Monomial basis only; less robust (Hankel assumption, division
  *                    by alpha_prev(s)).
+ *   "resident"     0 auto (default) | 1 off | 2 force.  The resident path runs the WHOLE loop of
+ *                  Alg. 3 in one cooperative launch: every CTA keeps its rows of the CSR arrays and of R, AR, P, AP, x, r
+ *                  in shared memory for the whole solve, s + 1 grid barriers per outer iteration instead of s + 2 kernel
+ *                  launches.  Auto picks it when every CTA's share fits shared memory (n up to a few 10^5 rows; the
+ *                  launch-bound regime, e.g. config 1), s <= 4 and form = 0; same arithmetic per row, same status codes.
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);
@@ -138,6 +143,13 @@ int sstep_cg_destroy(sstep_cg_t *handle);
 const char *sstep_cg_last_error(sstep_cg_t *handle);
 
 /* ---- test hooks: run exactly the production kernels on caller-supplied device buffers ---- */
+
+/* Copy one internal array of the current solve state to `out` (device, `count` doubles), after solve_begin / iterate:
+ * "R", "AR" (n*s, column-major: the basis blocks of the last MPK; R(:,1) already holds D^-1 r of the NEXT iteration),
+ * "P", "AP" (n*s, interleaved), "x", "r" (n), "M", "C", "W", "beta" (s*s, row-major), "m", "alpha" (s).
+ * Lets the parity tests check every stage of an outer iteration of the graph AND the resident path on identical
+ * inputs (the state before the iteration).  Synchronises the stream. */
+int sstep_cg_test_read_state(sstep_cg_t *handle, const char *name, double *out, int64_t count);
 
 /* a1, one SpMV of the matrix-powers kernel: y = A x; if yjac != NULL also yjac = D^-1 y. */
 int sstep_cg_test_spmv(sstep_cg_t *handle, const double *x, double *y, double *yjac);

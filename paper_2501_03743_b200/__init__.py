@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = [
     "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_profile_outer", "sstep_cg_solve_host", "sstep_cg_destroy",
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
     "sstep_cg_test_gram",
-    "sstep_cg_test_small_solve", "sstep_cg_test_update",
+    "sstep_cg_test_small_solve", "sstep_cg_test_update", "sstep_cg_test_read_state",
 ]
 
 
@@ -78,6 +78,7 @@ def load_library(build: bool = True):
     lib.sstep_cg_test_gram.argtypes = [vp] + [vp] * 7
     lib.sstep_cg_test_small_solve.argtypes = [vp] + [vp] * 8
     lib.sstep_cg_test_update.argtypes = [vp] + [vp] * 9
+    lib.sstep_cg_test_read_state.argtypes = [vp, C.c_char_p, vp, i64]
     for name in EXPORTED_SYMBOLS:
         if name != "sstep_cg_last_error":
             getattr(lib, name).restype = C.c_int
@@ -292,6 +293,17 @@ class SStepCG:
                                                         self._ptr(beta), self._ptr(alpha), self._ptr(W), self._ptr(st)),
                     "sstep_cg_test_small_solve")
         return int(st.item()), beta, alpha, W
+
+    def test_read_state(self, name: str):
+        """One internal array of the current solve state (see sstep_cg.h): blocks come back as (s, n) tensors."""
+        torch = _torch()
+        s, n = self.s, self.n
+        shape = {"R": (s, n), "AR": (s, n), "P": (n, s), "AP": (n, s), "x": (n,), "r": (n,), "M": (s, s), "C": (s, s),
+                 "W": (s, s), "beta": (s, s), "m": (s,), "alpha": (s,)}[name]
+        out = torch.empty(shape, dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._lib.sstep_cg_test_read_state(self._h, name.encode(), self._ptr(out), out.numel()),
+                    "sstep_cg_test_read_state")
+        return out.t().contiguous() if name in ("P", "AP") else out
 
     def test_update(self, R, AR, P, AP, x, r, beta, alpha):
         """Returns new (P, AP, x, r) as (s, n)/(n,) tensors plus R1 = D^-1 r_new and rho = ||r_new||^2; inputs are not modified."""

@@ -29,6 +29,11 @@ struct ScgState {
     unsigned int ticket_gram;
     unsigned int ticket_update;
     unsigned int ticket_init;
+    // grid barrier of the resident (cooperative) kernel, zeroed before each launch: arrival counter and, in another
+    // 128-byte line (the pollers must not queue behind the arriving atomics), the generation flag the last arriver sets
+    unsigned int grid_bar;
+    unsigned int grid_pad[31];
+    unsigned int grid_flag;
 };
 #define SCG_RUNNING (-1)
 

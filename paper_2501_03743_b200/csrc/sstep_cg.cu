@@ -11,6 +11,7 @@
 #include "gram.cuh"
 #include "gram_tma.cuh"
 #include "moment.cuh"
+#include "resident.cuh"
 #include "spmv.cuh"
 #include "update.cuh"
 #include "update_tma.cuh"
@@ -33,7 +34,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -59,6 +60,10 @@ struct sstep_cg {
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int64_t num_tiles = 0;
     int max_row_len = 0;
+    // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
+    bool resident = false;
+    int res_grid = 0, res_rpb = 0, res_nzcap = 0, res_threads = 0;
+    size_t res_smem = 0;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t gexec = nullptr;
     // host polling
@@ -281,6 +286,27 @@ cudaError_t launch_update(sstep_cg* h, cudaStream_t sm, bool configure, double* 
     SCG_DISPATCH_S(update_S, h, sm, configure, R, AR, P, AP, x, r, beta, alpha, st, rho_out)
 }
 
+// resident path (resident.cuh): op 0 = set the shared-memory attribute and report the occupancy, op 1 = cooperative launch
+template <int S>
+cudaError_t resident_S(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
+    if (op == 0) {
+        cudaError_t e = cudaFuncSetAttribute(resident_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->res_smem);
+        if (e != cudaSuccess) return e;
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_out, resident_kernel<S>, h->res_threads, h->res_smem);
+    }
+    ResidentParams p;
+    p.n = (int)h->n; p.rpb = h->res_rpb; p.nzcap = h->res_nzcap; p.kmax = kmax; p.basis = h->basis;
+    p.rp = h->rp; p.ci = h->ci; p.va = h->va; p.dinv = h->dinv;
+    p.Rg = h->R; p.ARg = h->AR; p.P = h->P; p.AP = h->AP; p.x = h->x; p.r = h->r;
+    p.partials = h->partials; p.st = h->st;
+    void* args[] = {&p};
+    return cudaLaunchCooperativeKernel((const void*)resident_kernel<S>, dim3(h->res_grid), dim3(h->res_threads), args, h->res_smem, sm);
+}
+
+cudaError_t resident_op(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
+    SCG_DISPATCH_S(resident_S, h, sm, op, kmax, occ_out)
+}
+
 // Alg. 4 on the given buffers: s Jacobi-fused SpMVs (R(:,1) must already hold D^-1 r)
 cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, const ScgState* st) {
     const int64_t n = h->n;
@@ -408,6 +434,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "spmv_depth" && value >= 2 && value <= 4) h->spmv_depth = (int)value;
     else if (k == "block_variant" && value >= 0 && value <= 2) h->block_variant = (int)value;
     else if (k == "form" && (value == 0 || value == 1)) h->form = (int)value;
+    else if (k == "resident" && value >= 0 && value <= 2) h->resident_opt = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -428,6 +455,10 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "kernels_per_outer") *value = kernels_per_outer(h);
     else if (k == "basis") *value = h->basis;
     else if (k == "launches") *value = h->launches;
+    else if (k == "resident") *value = h->resident ? 1 : 0;
+    else if (k == "resident_grid") *value = h->res_grid;
+    else if (k == "resident_rows_per_block") *value = h->res_rpb;
+    else if (k == "resident_smem_bytes") *value = (int64_t)h->res_smem;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown info key: " + k);
     return 0;
 }
@@ -506,6 +537,38 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         h->init_grid = (int)(want < cap ? want : cap);
     }
 
+    // resident path: whole loop in one cooperative launch when every CTA's rows fit shared memory
+    h->resident = false;
+    h->res_grid = 0;
+    // (auto: s <= 4 only -- above, the redundant per-CTA reduction of the 2s^2+s partials outweighs the saved launches)
+    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && n + 4096 < (int64_t(1) << 31)) {
+        int coop = 0;
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
+        int64_t g = (n + 31) / 32;
+        if (g > h->num_sms) g = h->num_sms;
+        int64_t rpb = ((n + g - 1) / g + 31) / 32 * 32;
+        g = (n + rpb - 1) / rpb;
+        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
+        tile_nnz_max_kernel<<<(unsigned)((g + 255) / 256), 256, 0, sm>>>(n, rowptr, (int)rpb, g, h->iscratch + 3);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        const int nzcap = (hs[3] + 3) & ~3;
+        const size_t bytes = resident_smem_bytes(s, (int)rpb, nzcap);
+        if (coop && bytes <= (size_t)200 * 1024) {
+            h->res_grid = (int)g; h->res_rpb = (int)rpb; h->res_nzcap = nzcap; h->res_smem = bytes;
+            h->res_threads = (int)(rpb < 512 ? rpb : 512);
+            int occ = 0;
+            CK(resident_op(h, sm, 0, 0, &occ));
+            h->resident = occ >= 1 && (int64_t)occ * h->num_sms >= g;
+        }
+        if (!h->resident) h->res_grid = 0;
+    }
+    if (h->resident_opt == 2 && !h->resident) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: resident path forced but the problem does not fit shared memory (or form = 1)");
+    }
+
     // workspaces
     const size_t blk = sizeof(double) * (size_t)n * s;
     CK(cudaMalloc(&h->R, blk));
@@ -517,6 +580,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     size_t np = (size_t)h->gram_grid * (2 * s * s + s);
     if (np < 2 * (size_t)h->update_grid) np = 2 * (size_t)h->update_grid;
     if (np < 2 * (size_t)h->init_grid) np = 2 * (size_t)h->init_grid;
+    if (np < (size_t)h->res_grid * (2 * s * s + s + 1)) np = (size_t)h->res_grid * (2 * s * s + s + 1);
     CK(cudaMalloc(&h->partials, sizeof(double) * np));
     CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
     CK(cudaMemsetAsync(h->mom, 0, sizeof(double) * 2 * s * (size_t)h->spmv_grid, sm));
@@ -569,6 +633,14 @@ int sstep_cg_solve_begin(sstep_cg_t* h, const double* b, const double* x0, doubl
 int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
     if (!h || k_outer < 0) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "iterate: call solve_begin first");
+    if (h->resident) {  // one cooperative launch runs up to k_outer outer iterations (stops on the device at convergence)
+        if (k_outer == 0) return 0;
+        CK(cudaMemsetAsync(&h->st->grid_bar, 0, 33 * sizeof(unsigned int), h->stream));
+        CK(resident_op(h, h->stream, 1, k_outer, nullptr));
+        h->launches++;
+        h->graph_launches++;
+        return 0;
+    }
     for (int i = 0; i < k_outer; i++) {
         if (h->use_graph) {
             CK(cudaGraphLaunch(h->gexec, h->stream));
@@ -584,6 +656,7 @@ int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
 int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
     if (!h || reps < 1 || !ms_host) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "profile_outer: call solve_begin first");
+    if (h->resident) return fail(h, SSTEP_CG_ERR_STATE, "profile_outer: the resident path has no per-kernel launches (set option resident = 1)");
     cudaStream_t sm = h->stream;
     const int per = h->s + 2;
     const int nev = reps * per * 2;
@@ -663,6 +736,11 @@ int sstep_cg_solve(sstep_cg_t* h, const double* b, const double* x0, double* x, 
     int rc = sstep_cg_solve_begin(h, b, x0, rtol);
     if (rc) return rc;
     cudaStream_t sm = h->stream;
+    if (h->resident) {  // the whole loop is one launch; the stop test runs on the device
+        rc = sstep_cg_iterate(h, maxit);
+        if (rc) return rc;
+        return sstep_cg_solve_end(h, x, out);
+    }
     // Replay the outer-iteration graph in chunks; two chunks are kept in flight so the device never waits for the
     // host.  Iterations enqueued after convergence exit on the device flag (a few microseconds each).
     const int chunk = h->n >= (int64_t(1) << 21) ? 2 : 8;
@@ -732,6 +810,33 @@ static int hook_prepare(sstep_cg* h) {
     memset(&init, 0, sizeof init);
     init.status = SCG_RUNNING;
     CK(cudaMemcpyAsync(h->st_test, &init, sizeof(Header) /* header only; tickets stay 0 */, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_read_state(sstep_cg_t* h, const char* name, double* out, int64_t count) {
+    if (!h || !name || !out) return SSTEP_CG_ERR_ARG;
+    if (!h->ready) return fail(h, SSTEP_CG_ERR_STATE, "test_read_state: call setup first");
+    CK(cudaSetDevice(h->device));
+    const std::string k(name);
+    const int64_t ns = h->n * h->s, ss = (int64_t)h->s * h->s;
+    const double* src = nullptr;
+    int64_t want = 0;
+    if (k == "R") { src = h->R; want = ns; }
+    else if (k == "AR") { src = h->AR; want = ns; }
+    else if (k == "P") { src = h->P; want = ns; }
+    else if (k == "AP") { src = h->AP; want = ns; }
+    else if (k == "x") { src = h->x; want = h->n; }
+    else if (k == "r") { src = h->r; want = h->n; }
+    else if (k == "M") { src = h->st->M; want = ss; }
+    else if (k == "C") { src = h->st->C; want = ss; }
+    else if (k == "W") { src = h->st->W; want = ss; }
+    else if (k == "beta") { src = h->st->beta; want = ss; }
+    else if (k == "m") { src = h->st->m; want = h->s; }
+    else if (k == "alpha") { src = h->st->alpha; want = h->s; }
+    else return fail(h, SSTEP_CG_ERR_ARG, "test_read_state: unknown array " + k);
+    if (count != want) return fail(h, SSTEP_CG_ERR_ARG, "test_read_state: wrong element count for " + k);
+    CK(cudaMemcpyAsync(out, src, sizeof(double) * want, cudaMemcpyDeviceToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return 0;
 }

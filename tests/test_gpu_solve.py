@@ -1,4 +1,5 @@
-"""End-to-end GPU parity: sstep_cg_solve (graph-captured loop, device-side stop test) against the oracle's
+"""End-to-end GPU parity: sstep_cg_solve (graph-captured loop, device-side stop test; option resident = 1 keeps these
+small systems on the graph path -- the resident path has its own file, test_gpu_resident.py) against the oracle's
 Alg. 3 (Gram form) on the BASELINE.json configs, at sizes the oracle finishes in seconds, plus the edge and
 degenerate cases.  Bars (north_star): final solution relative difference <= 1e-8, outer iterations within +-1.
 s = 8 with the paper's monomial basis is "parity unpinned" end to end: there the test enforces
@@ -30,6 +31,7 @@ def dev(torch, a):
 
 
 def gpu_solve(cg, torch, c, s, rtol, maxit, x0=None, **opts):
+    opts.setdefault("resident", 1)
     with cg.SStepCG(0, **opts) as h:
         h.setup(dev(torch, c["rowptr"]), dev(torch, c["colidx"]), dev(torch, c["vals"]), s)
         x, res = h.solve(dev(torch, c["b"]), None if x0 is None else dev(torch, x0), rtol=rtol, maxit=maxit)
@@ -104,7 +106,7 @@ def test_iterate_trajectory_matches_oracle(oracle_mod, cg_mod, torch_mod):
     """solve_begin / iterate(k) / solve_end: iterate i equals the oracle's iterate i (early iterations, s = 3)."""
     c = gen.make_config(2, N=20)
     ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 3, rtol=0.0, maxit=6, xhist_cap=6, history=True)
-    with cg_mod.SStepCG(0) as h:
+    with cg_mod.SStepCG(0, resident=1) as h:
         h.setup(dev(torch_mod, c["rowptr"]), dev(torch_mod, c["colidx"]), dev(torch_mod, c["vals"]), 3)
         b = dev(torch_mod, c["b"])
         for k in range(1, 7):
@@ -127,7 +129,7 @@ def test_s1_pipeline_is_the_papers_fcg_comparator(oracle_mod, cg_mod, torch_mod,
     rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
     ref2 = oracle_mod.pfcg(rp, ci, v, b, rtol=0.0, maxit=8, xhist_cap=8)
     ref1 = oracle_mod.pcg(rp, ci, v, b, rtol=0.0, maxit=8, xhist_cap=8)
-    with cg_mod.SStepCG(0, form=form) as h:
+    with cg_mod.SStepCG(0, form=form, resident=1) as h:
         h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), 1)
         bd = dev(torch_mod, b)
         for k in (1, 2, 5, 8):
