@@ -221,8 +221,13 @@ def run_ours(args):
     moment = {}
     for form, s in runs:
         with cg.SStepCG(local, form=form, resident=1) as h:      # graph path: one launch per kernel, per-kernel times
+            torch.cuda.synchronize()
+            t_setup = time.perf_counter()
             h.setup(rp, ci, va, s)
-            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid")}
+            torch.cuda.synchronize()
+            t_setup = time.perf_counter() - t_setup
+            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid", "reordered", "cm_levels")}
+            info["setup_seconds"] = t_setup      # validation, dinv, (auto) Cuthill-McKee reordering, workspaces, graph capture
             if s == s0 and form == 0:
                 with ClockSampler(local) as clk:
                     ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)

@@ -102,6 +102,13 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  in shared memory for the whole solve, s + 1 grid barriers per outer iteration instead of s + 2 kernel
  *                  launches.  Auto picks it when every CTA's share fits shared memory (n up to a few 10^5 rows; the
  *                  launch-bound regime, e.g. config 1), s <= 4 and form = 0; same arithmetic per row, same status codes.
+ *   "reorder"      0 auto (default) | 1 off | 2 force.  Setup-time symmetric reordering A' = Pi A Pi^T for gather locality
+ *                  (Cuthill-McKee numbering computed on the device, csrc/reorder.cuh); the solver then owns a permuted
+ *                  copy of the CSR arrays, permutes b and x0 on the way in and x on the way out.  In exact arithmetic
+ *                  every iterate is unchanged (the Jacobi preconditioner commutes with Pi); in fp64 only the order of
+ *                  the Gram sums changes.  Auto: n >= 2^23 rows (the gathered vector cannot live in L2) and more than a
+ *                  quarter of the entries further than 2^20 rows from the diagonal (e.g. config 5's randomly permuted
+ *                  rows, where every 8-byte gather otherwise costs a 64-byte DRAM access).
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);
@@ -141,6 +148,12 @@ int sstep_cg_destroy(sstep_cg_t *handle);
 
 /* Text of the last failure on this handle ("" if none).  Never NULL. */
 const char *sstep_cg_last_error(sstep_cg_t *handle);
+
+/* The row numbering the solver works in: perm_out[i'] (device, n int32) = the caller's index of the solver's row i'
+ * (the identity unless setup reordered the matrix, option "reorder").  sstep_cg_solve / solve_begin / solve_end /
+ * solve_host take and return vectors in the CALLER's numbering; the test hooks below and sstep_cg_test_read_state
+ * work in the SOLVER's numbering (v'[i'] = v[perm[i']]). */
+int sstep_cg_get_permutation(sstep_cg_t *handle, int32_t *perm_out);
 
 /* ---- test hooks: run exactly the production kernels on caller-supplied device buffers ---- */
 

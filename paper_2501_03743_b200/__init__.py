@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = [
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
     "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update", "sstep_cg_test_read_state",
+    "sstep_cg_get_permutation",
 ]
 
 
@@ -79,6 +80,7 @@ def load_library(build: bool = True):
     lib.sstep_cg_test_small_solve.argtypes = [vp] + [vp] * 8
     lib.sstep_cg_test_update.argtypes = [vp] + [vp] * 9
     lib.sstep_cg_test_read_state.argtypes = [vp, C.c_char_p, vp, i64]
+    lib.sstep_cg_get_permutation.argtypes = [vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name != "sstep_cg_last_error":
             getattr(lib, name).restype = C.c_int
@@ -169,6 +171,13 @@ class SStepCG:
                     "sstep_cg_setup")
         self._keep = [rowptr, colidx, vals]  # borrowed by the library until the next setup / destroy
         self.n, self.nnz, self.s = n, nnz, int(s)
+
+    def get_permutation(self):
+        """perm[i'] = the caller's index of the solver's row i' (identity unless setup reordered the matrix)."""
+        torch = _torch()
+        perm = torch.empty(self.n, dtype=torch.int32, device=f"cuda:{self.device}")
+        self._check(self._lib.sstep_cg_get_permutation(self._h, self._ptr(perm)), "sstep_cg_get_permutation")
+        return perm
 
     def solve(self, b, x0=None, rtol: float = 1e-8, maxit: int = 2000):
         torch = _torch()

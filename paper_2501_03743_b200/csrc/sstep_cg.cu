@@ -11,6 +11,7 @@
 #include "gram.cuh"
 #include "gram_tma.cuh"
 #include "moment.cuh"
+#include "reorder.cuh"
 #include "resident.cuh"
 #include "spmv.cuh"
 #include "update.cuh"
@@ -34,7 +35,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -60,6 +61,12 @@ struct sstep_cg {
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int64_t num_tiles = 0;
     int max_row_len = 0;
+    // locality reordering (reorder.cuh): A' = Pi A Pi^T in owned arrays; rp/ci/va above then point at them
+    bool reordered = false;
+    int *perm = nullptr, *rank = nullptr;        // perm[new] = old, rank[old] = new
+    int *own_prp = nullptr, *own_pci = nullptr;
+    double *own_pva = nullptr, *bperm = nullptr, *x0perm = nullptr;
+    int cm_levels = 0, cm_comps = 0, far_permille = 0;
     // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
     bool resident = false;
     int res_grid = 0, res_rpb = 0, res_nzcap = 0, res_threads = 0;
@@ -353,6 +360,17 @@ void free_problem(sstep_cg* h) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
+    int** ibufs[] = {&h->perm, &h->rank, &h->own_prp, &h->own_pci};
+    for (int** b : ibufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    double** dbufs[] = {&h->own_pva, &h->bperm, &h->x0perm};
+    for (double** b : dbufs) {
+        if (*b) cudaFree(*b);
+        *b = nullptr;
+    }
+    h->reordered = false;
     h->ready = false;
     h->in_solve = false;
 }
@@ -368,6 +386,11 @@ void free_owned(sstep_cg* h) {
 }
 
 int kernels_per_outer(const sstep_cg* h) { return h->s + 2; }
+
+__global__ void iota_kernel(int64_t n, int* __restrict__ p) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = (int)i;
+}
 
 }  // namespace
 
@@ -435,6 +458,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "block_variant" && value >= 0 && value <= 2) h->block_variant = (int)value;
     else if (k == "form" && (value == 0 || value == 1)) h->form = (int)value;
     else if (k == "resident" && value >= 0 && value <= 2) h->resident_opt = (int)value;
+    else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -455,6 +479,10 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "kernels_per_outer") *value = kernels_per_outer(h);
     else if (k == "basis") *value = h->basis;
     else if (k == "launches") *value = h->launches;
+    else if (k == "reordered") *value = h->reordered ? 1 : 0;
+    else if (k == "cm_levels") *value = h->cm_levels;
+    else if (k == "cm_components") *value = h->cm_comps;
+    else if (k == "far_permille") *value = h->far_permille;
     else if (k == "resident") *value = h->resident ? 1 : 0;
     else if (k == "resident_grid") *value = h->res_grid;
     else if (k == "resident_rows_per_block") *value = h->res_rpb;
@@ -493,6 +521,52 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         return fail(h, SSTEP_CG_ERR_MATRIX, buf);
     }
     h->max_row_len = hs[1];
+
+    // locality reordering (reorder.cuh).  auto: only when the gathered vector cannot live in L2 (n >= 2^23 rows = 67 MB)
+    // and more than a quarter of the entries reach further than 2^20 rows (8 MB) from the diagonal.
+    {
+        unsigned long long* far = nullptr;
+        unsigned long long hfar = 0;
+        CK(cudaMalloc(&far, sizeof(unsigned long long)));
+        CK(cudaMemsetAsync(far, 0, sizeof(unsigned long long), sm));
+        scg_reorder::far_entries_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, 1 << 20, far);
+        CK(cudaMemcpyAsync(&hfar, far, sizeof(unsigned long long), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        cudaFree(far);
+        h->far_permille = (int)(1000.0 * (double)hfar / (double)nnz);
+    }
+    h->cm_levels = h->cm_comps = 0;
+    if (h->reorder_opt == 2 || (h->reorder_opt == 0 && n >= (int64_t(1) << 23) && h->far_permille > 250)) {
+        CK(cudaMalloc(&h->perm, sizeof(int) * (size_t)n));
+        CK(cudaMalloc(&h->rank, sizeof(int) * (size_t)n));
+        bool done = false;
+        CK(scg_reorder::cuthill_mckee((int)n, rowptr, colidx, sm, h->perm, h->rank, &done, &h->cm_levels, &h->cm_comps));
+        if (done) {
+            CK(cudaMalloc(&h->own_prp, sizeof(int) * ((size_t)n + 1)));
+            CK(cudaMalloc(&h->own_pci, sizeof(int) * (size_t)nnz));
+            CK(cudaMalloc(&h->own_pva, sizeof(double) * (size_t)nnz));
+            CK(cudaMalloc(&h->bperm, sizeof(double) * (size_t)n));
+            CK(cudaMalloc(&h->x0perm, sizeof(double) * (size_t)n));
+            CK(scg_reorder::permute_csr((int)n, (int)nnz, h->perm, h->rank, rowptr, colidx, vals, h->own_prp, h->own_pci, h->own_pva, sm));
+            h->rp = rowptr = h->own_prp;
+            h->ci = colidx = h->own_pci;
+            h->va = vals = h->own_pva;
+            h->reordered = true;
+            // dinv and the row statistics of the permuted matrix (same validation, now of our own copy)
+            CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
+            analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+            if (hs[0]) {
+                free_problem(h);
+                return fail(h, SSTEP_CG_ERR_CUDA, "setup: internal error, the permuted matrix failed validation");
+            }
+        } else {  // too many connected components: keep the caller's numbering
+            cudaFree(h->perm); cudaFree(h->rank);
+            h->perm = h->rank = nullptr;
+        }
+    }
 
     // SpMV variant: lanes per row from the mean row length (vector-per-row ... warp-per-row), bulk staging if every tile fits
     const double mean = (double)nnz / (double)n;
@@ -620,6 +694,16 @@ int sstep_cg_solve_begin(sstep_cg_t* h, const double* b, const double* x0, doubl
     const size_t blk = sizeof(double) * (size_t)h->n * h->s;
     CK(cudaMemsetAsync(h->P, 0, blk, sm));
     CK(cudaMemsetAsync(h->AP, 0, blk, sm));
+    if (h->reordered) {  // b' = Pi b, x0' = Pi x0
+        const unsigned g = (unsigned)((h->n + 255) / 256);
+        scg_reorder::gather_vec_kernel<<<g, 256, 0, sm>>>(h->n, h->perm, b, h->bperm);
+        b = h->bperm;
+        if (x0) {
+            scg_reorder::gather_vec_kernel<<<g, 256, 0, sm>>>(h->n, h->perm, x0, h->x0perm);
+            x0 = h->x0perm;
+        }
+        CK(cudaGetLastError());
+    }
     if (x0) {  // r <- A x0 with the production SpMV, then r <- b - r in init_kernel
         CK(launch_spmv(h, sm, x0, h->r, nullptr, nullptr, 0, nullptr));
     }
@@ -713,7 +797,12 @@ int sstep_cg_solve_end(sstep_cg_t* h, double* x, sstep_cg_result* out) {
     if (!h) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "solve_end: call solve_begin first");
     cudaStream_t sm = h->stream;
-    if (x) CK(cudaMemcpyAsync(x, h->x, sizeof(double) * h->n, cudaMemcpyDeviceToDevice, sm));
+    if (x && h->reordered) {  // x = Pi^T x'
+        scg_reorder::scatter_vec_kernel<<<(unsigned)((h->n + 255) / 256), 256, 0, sm>>>(h->n, h->perm, h->x, x);
+        CK(cudaGetLastError());
+    } else if (x) {
+        CK(cudaMemcpyAsync(x, h->x, sizeof(double) * h->n, cudaMemcpyDeviceToDevice, sm));
+    }
     CK(cudaMemcpyAsync(&h->h_hdr[0], h->st, sizeof(Header), cudaMemcpyDeviceToHost, sm));
     CK(cudaStreamSynchronize(sm));
     h->in_solve = false;
@@ -810,6 +899,20 @@ static int hook_prepare(sstep_cg* h) {
     memset(&init, 0, sizeof init);
     init.status = SCG_RUNNING;
     CK(cudaMemcpyAsync(h->st_test, &init, sizeof(Header) /* header only; tickets stay 0 */, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_get_permutation(sstep_cg_t* h, int32_t* perm_out) {
+    if (!h || !perm_out) return SSTEP_CG_ERR_ARG;
+    if (!h->ready) return fail(h, SSTEP_CG_ERR_STATE, "get_permutation: call setup first");
+    CK(cudaSetDevice(h->device));
+    if (h->reordered) {
+        CK(cudaMemcpyAsync(perm_out, h->perm, sizeof(int) * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+        iota_kernel<<<(unsigned)((h->n + 255) / 256), 256, 0, h->stream>>>(h->n, perm_out);
+        CK(cudaGetLastError());
+    }
     CK(cudaStreamSynchronize(h->stream));
     return 0;
 }
