@@ -281,13 +281,15 @@ def run_ours(args):
 
 
 def run_e2e(args, ctx):
-    """The same metric through the C-ABI call with HOST buffers: H2D of CSR + b, setup, k outer iterations,
-    D2H of x, all inside the timed region."""
+    """The same metric through the C-ABI call with HOST buffers, as a user makes it: ONE sstep_cg_solve_host call that
+    uploads the pinned CSR arrays and b, runs setup and the WHOLE solve to the config's own tolerance (config 4:
+    rtol = 1e-8, 125 outer iterations at s = 4) and downloads x -- all inside the timed region.  value = that time
+    divided by the outer iterations executed."""
     import torch
 
     import paper_2501_03743_b200 as cg
     c, s = ctx["c"], args.s
-    k = min(args.steps, restart_every_for(s))
+    rtol = float(c.get("rtol", 1e-8))
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     rp, ci, va, b = pin(c["rowptr"]), pin(c["colidx"]), pin(c["vals"]), pin(c["b"])
     x = torch.empty(c["n"], dtype=torch.float64).pin_memory()
@@ -298,16 +300,24 @@ def run_e2e(args, ctx):
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             ev0.record()
-            _, res = h.solve_host(rp, ci, va, b, s, rtol=0.0, maxit=k, x_out=x)
+            _, res = h.solve_host(rp, ci, va, b, s, rtol=rtol, maxit=2000, x_out=x)
             ev1.record()
             torch.cuda.synchronize()
             wall_ms = 1e3 * (time.perf_counter() - t0)
             best = dict(ms=max(ev0.elapsed_time(ev1), wall_ms), res=res)
-    assert best["res"]["outer_iters"] == k and best["res"]["status"] == 1
+    k = best["res"]["outer_iters"]
+    assert k >= 1 and best["res"]["status"] in (0, 1, 2), best
+    xerr = None
+    if "xstar" in c and c["xstar"] is not None:
+        xs = np.asarray(c["xstar"])
+        xerr = float(np.linalg.norm(x.numpy() - xs) / np.linalg.norm(xs))
     h2d = rp.numel() * 4 + ci.numel() * 4 + va.numel() * 8 + b.numel() * 8
     return dict(value=1e3 * best["ms"] / k, unit="us", h2d_bytes_per_step=h2d / k, d2h_bytes_per_step=x.numel() * 8 / k,
-                outer_iters=k, note="one sstep_cg_solve_host call: pinned host CSR+b -> device, setup (dinv, graph capture), "
-                                    f"{k} outer iterations, x -> host; all inside the timed region")
+                outer_iters=k, status=best["res"]["status_name"], relres=best["res"]["relres"], rtol=rtol, total_ms=best["ms"],
+                rel_error_vs_xstar=xerr,
+                note="one sstep_cg_solve_host call: pinned host CSR+b -> device, setup (validation, dinv, reordering if "
+                     f"needed, graph capture), the whole solve to rtol={rtol:g} ({k} outer iterations), x -> host; all "
+                     "inside the timed region; value = total / outer iterations")
 
 
 def run_cpu_baseline(args, ctx):
