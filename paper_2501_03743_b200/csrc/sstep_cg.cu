@@ -24,8 +24,13 @@ struct Header {  // mirrors the first fields of ScgState
     double rho, rho0, rtol;
 };
 
+// bulk-staged SpMV shapes: nnz capacity of one warp tile / warps per CTA.  256 x 8 is the thread-per-row shape of the
+// 7-point configs; the two larger tiles keep FEW lanes per row for longer rows (27-point: L = 2 -> 16 rows x 27, L = 1 ->
+// 32 rows x 27 per tile), because consecutive rows under the same lane index gather consecutive x entries.
 constexpr int BULK_CAP = 256, BULK_WPC = 8;
-constexpr size_t bulk_smem(int D) { return (size_t)BULK_WPC * D * BULK_CAP * 12 + (size_t)BULK_WPC * D * 8; }
+constexpr int BULK_CAP2 = 512, BULK_WPC2 = 8;     // L = 2, depth 2
+constexpr int BULK_CAP1 = 1024, BULK_WPC1 = 4;    // L = 1, depth 2
+constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D * cap * 12 + (size_t)wpc * D * 8; }
 
 }  // namespace
 
@@ -56,6 +61,7 @@ struct sstep_cg {
     // kernel configuration
     int lanes = 1;
     bool bulk = false;
+    int bulk_cap = 256, bulk_wpc = 8;
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0;
     bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
@@ -111,13 +117,21 @@ bulk_fn_t bulk_kernel_mom(int depth) {
     }
 }
 template <int L>
-bulk_fn_t bulk_kernel_for(int depth, bool mom) { return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth); }
+bulk_fn_t bulk_kernel_for(int depth, bool mom, int cap) {
+    if constexpr (L == 1) {
+        if (cap == BULK_CAP1) return mom ? spmv_bulk_kernel<1, 2, BULK_CAP1, BULK_WPC1, true, 2> : spmv_bulk_kernel<1, 2, BULK_CAP1, BULK_WPC1, false, 2>;
+    }
+    if constexpr (L == 2) {
+        if (cap == BULK_CAP2) return mom ? spmv_bulk_kernel<2, 2, BULK_CAP2, BULK_WPC2, true, 2> : spmv_bulk_kernel<2, 2, BULK_CAP2, BULK_WPC2, false, 2>;
+    }
+    return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth);
+}
 
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if (h->bulk) {
-        bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr)<<<h->spmv_grid, BULK_WPC * 32, bulk_smem(h->spmv_depth), sm>>>(
+        bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr, h->bulk_cap)<<<h->spmv_grid, h->bulk_wpc * 32, bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc), sm>>>(
             (int)h->n, (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, (int)h->num_tiles, mom_a, mom_b);
     } else {
         if (mom_a) spmv_vec_kernel<L, true><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
@@ -144,17 +158,17 @@ cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
     if (h->bulk) {
-        auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0);
-        const size_t smem = bulk_smem(h->spmv_depth);
+        auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0, h->bulk_cap);
+        const size_t smem = bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc);
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         // (the variant without moments is also launched in the moment form: x0 != 0 start-up, test_spmv hook)
-        e = cudaFuncSetAttribute(bulk_kernel_for<L>(h->spmv_depth, false), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(bulk_kernel_for<L>(h->spmv_depth, false, h->bulk_cap), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, BULK_WPC * 32, smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, h->bulk_wpc * 32, smem);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
-        int64_t want = (h->num_tiles + BULK_WPC - 1) / BULK_WPC;
+        int64_t want = (h->num_tiles + h->bulk_wpc - 1) / h->bulk_wpc;
         int64_t cap = (int64_t)occ * h->num_sms;
         h->spmv_grid = (int)(want < cap ? want : cap);
     } else {
@@ -576,9 +590,12 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     h->bulk = false;
     const bool aligned = (((uintptr_t)colidx | (uintptr_t)vals) & 15) == 0;
     // auto: the bulk-staged kernel for thread-per-row matrices (mean row <= 8 entries, e.g. 7-point stencils), where it
-    // reaches ~95 % of the copy peak; with several lanes per row the generic kernel is faster (27-point 160^3: 269 vs
-    // 356 us).  Forced (spmv_variant = 2): any L whose tiles fit.
-    if ((h->spmv_variant == 2 || (h->spmv_variant == 0 && L == 1)) && aligned && n + 64 < (int64_t(1) << 31)) {
+    // reaches the copy peak, and -- with TWO lanes per row and 512-entry tiles -- for mean rows of 16..32 entries
+    // (27-point 160^3: 257 us against 272 us for the generic kernel at L = 4 and 285 us for bulk tiles at L = 4: few lanes
+    // per row keep the x gathers of a warp on consecutive addresses).  Forced (spmv_variant = 2): any L whose tiles fit.
+    const bool auto_bulk = h->spmv_variant == 0 && (L == 1 || (L == 4 && !h->lanes_opt && h->spmv_depth == 2));
+    if ((h->spmv_variant == 2 || auto_bulk) && aligned && n + 64 < (int64_t(1) << 31)) {
+        if (auto_bulk && L == 4) L = 2;
         for (int Lb = L; Lb <= 32; Lb *= 2) {
             const int rpt = 32 / Lb;
             const int64_t tiles = (n + rpt - 1) / rpt;
@@ -587,14 +604,21 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
             CK(cudaGetLastError());
             CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
             CK(cudaStreamSynchronize(sm));
-            if (hs[2] + 3 <= BULK_CAP) {
+            int cap = 0, wpc = BULK_WPC;
+            if (hs[2] + 3 <= BULK_CAP) cap = BULK_CAP;
+            else if (Lb == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP2) { cap = BULK_CAP2; wpc = BULK_WPC2; }
+            else if (Lb == 1 && h->spmv_variant == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP1) { cap = BULK_CAP1; wpc = BULK_WPC1; }
+            if (cap) {
                 h->bulk = true;
+                h->bulk_cap = cap;
+                h->bulk_wpc = wpc;
                 L = Lb;
                 h->num_tiles = tiles;
                 break;
             }
             if (h->lanes_opt || h->spmv_variant == 0) break;
         }
+        if (auto_bulk && !h->bulk && L == 2) L = 4;  // tiles too large: back to the generic kernel at its own L
     }
     if (h->spmv_variant == 2 && !h->bulk) {
         free_problem(h);
