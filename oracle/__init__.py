@@ -184,9 +184,13 @@ def pfcg(rowptr, colidx, vals, b, x0=None, rtol=1e-8, maxit=2000, history=False,
 
 
 def sstep(rowptr, colidx, vals, b, s, x0=None, rtol=1e-8, maxit=2000, form="gram", basis=0,
-          history=False, xhist_cap=0):
+          history=False, xhist_cap=0, replace_every=0):
     """Alg. 3 PCGs; form 'gram' (O2), 'moment' (O3, Alg. 5 + Alg. 6) or 'moment_fused' (O3 with the moments taken
-    in the MPK, cvm_fused); iters = outer iterations."""
+    in the MPK, cvm_fused); iters = outer iterations.  replace_every = R > 0: residual replacement every R outer
+    iterations (orc_sstep_rr; with history, hist[k] is the replaced residual on those iterations)."""
     f = {"gram": 0, "moment": 1, "moment_fused": 2}[form]
+    if replace_every:
+        return _solver_common(lib().orc_sstep_rr, rowptr, colidx, vals, b, x0, rtol, maxit,
+                              (C.c_int(s), C.c_int(f), C.c_int(basis), C.c_int(replace_every)), history, xhist_cap)
     return _solver_common(lib().orc_sstep, rowptr, colidx, vals, b, x0, rtol, maxit,
                           (C.c_int(s), C.c_int(f), C.c_int(basis)), history, xhist_cap)

@@ -402,9 +402,13 @@ done:
  *   form = 1: paper-literal moment form (O3): orc_cvm (Alg. 5) + orc_sw (Alg. 6)
  * maxit counts OUTER iterations (reading A9); *iters = outer iterations done.
  */
-int orc_sstep(i64 n, const i32 *rp, const i32 *ci, const double *v, const double *b,
-              const double *x0, int s, int form, int basis, double rtol, int maxit, double *x,
-              int *iters, double *relres, double *hist, double *xhist, int xhist_cap)
+/* replace_every = R > 0: residual replacement (related work; reading A22 of DESIGN.md).  After the block
+ * update of every R-th outer iteration -- unless the recurrence residual has just passed the stop test -- r is
+ * overwritten by the true residual b - A x (one extra SpMV), the directions P, AP are kept, and the stop test is taken
+ * again on the replaced residual; hist[k] then holds the replaced value.  R = 0: never (Alg. 3 as printed). */
+int orc_sstep_rr(i64 n, const i32 *rp, const i32 *ci, const double *v, const double *b,
+                 const double *x0, int s, int form, int basis, int replace_every, double rtol, int maxit, double *x,
+                 int *iters, double *relres, double *hist, double *xhist, int xhist_cap)
 {
     if (s < 1 || s > ORC_SMAX) return -1;
     size_t blk = sizeof(double) * (size_t)n * s;
@@ -450,8 +454,24 @@ int orc_sstep(i64 n, const i32 *rp, const i32 *ci, const double *v, const double
         if (xhist && k < xhist_cap) memcpy(xhist + (i64)k * n, x, sizeof(double) * n);
         if (!isfinite(nr)) { status = 2; break; }
         if (nr < rtol * nr0) { status = 0; break; }                    /* l.31-33 */
+        if (replace_every > 0 && (k + 1) % replace_every == 0) {
+            orc_spmv(n, rp, ci, v, x, R);                              /* R(:,1) is scratch here: the next MPK rewrites it */
+            for (i64 i = 0; i < n; i++) r[i] = b[i] - R[i];
+            nr = sqrt((double)ldot(n, r, r));
+            *relres = nr / nr0;
+            if (hist) hist[k] = *relres;
+            if (!isfinite(nr)) { status = 2; break; }
+            if (nr < rtol * nr0) { status = 0; break; }
+        }
     }
 done:
     free(r); free(dinv); free(R); free(AR); free(P); free(AP);
     return status;
+}
+
+int orc_sstep(i64 n, const i32 *rp, const i32 *ci, const double *v, const double *b,
+              const double *x0, int s, int form, int basis, double rtol, int maxit, double *x,
+              int *iters, double *relres, double *hist, double *xhist, int xhist_cap)
+{
+    return orc_sstep_rr(n, rp, ci, v, b, x0, s, form, basis, 0, rtol, maxit, x, iters, relres, hist, xhist, xhist_cap);
 }

@@ -194,6 +194,48 @@ def test_status_codes(oracle_mod):
     assert a["status"] == 0 and np.linalg.norm(a["x"] - c["xstar"]) <= 1e-8 * np.linalg.norm(c["xstar"])
 
 
+# residual replacement (reading A22) -----------------------
+@pytest.mark.parametrize("s,R", [(1, 3), (2, 1), (3, 2), (4, 5)])
+def test_residual_replacement_pins(oracle_mod, s, R):
+    """What fixes orc_sstep_rr without an implementation to compare with: (i) R beyond the iteration count changes
+    nothing, bit for bit; (ii) on a replacement iteration the reported residual IS the true residual of that iterate
+    (recomputed here with scipy's CSR product); on the others it is the recurrence residual, which drifts from the
+    true one; (iii) replacing r by b - A x changes r only at rounding level, so the early iterates agree with the
+    unreplaced ones; (iv) it still converges to the dense-LU solution."""
+    c = gen.make_config(2, N=10)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    A = csr_of(c)
+    nb = np.linalg.norm(b)
+    plain = oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-10, maxit=200, history=True, xhist_cap=200)
+    never = oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-10, maxit=200, history=True, xhist_cap=200, replace_every=10 ** 6)
+    assert never["iters"] == plain["iters"] and np.array_equal(never["x"], plain["x"]) and np.array_equal(never["hist"], plain["hist"])
+    rr = oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-10, maxit=200, history=True, xhist_cap=200, replace_every=R)
+    assert rr["status"] == 0 and abs(rr["iters"] - plain["iters"]) <= 1
+    for k in range(rr["iters"]):
+        true = np.linalg.norm(b - A @ rr["xhist"][k]) / nb
+        if (k + 1) % R == 0:
+            assert abs(rr["hist"][k] - true) <= 1e-13 * max(true, 1e-16 / nb) + 1e-15, k
+    for k in range(min(4, plain["iters"], rr["iters"])):
+        assert np.linalg.norm(rr["xhist"][k] - plain["xhist"][k]) <= 1e-12 * np.linalg.norm(plain["xhist"][k])
+    xs = np.linalg.solve(A.toarray(), b)
+    assert np.linalg.norm(rr["x"] - xs) <= 1e-8 * np.linalg.norm(xs)
+
+
+def test_residual_replacement_reports_the_true_residual_at_the_accuracy_limit(oracle_mod):
+    """Run past the attainable accuracy (rtol = 0) with replacement every iteration: the reported residual stays the
+    true residual of the iterate (it cannot drift below what fp64 allows -- the reason the technique exists,
+    PAPER.md:251) and the iterate stays at the accuracy limit instead of wandering off."""
+    c = gen.make_config(2, N=8)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    A = csr_of(c)
+    nb = np.linalg.norm(b)
+    rr = oracle_mod.sstep(rp, ci, v, b, 2, rtol=0.0, maxit=40, history=True, replace_every=1)
+    n_rr = rr["iters"]
+    assert n_rr >= 20
+    true = np.linalg.norm(b - A @ rr["x"]) / nb
+    assert abs(rr["hist"][n_rr - 1] - true) <= 1e-12 * true + 1e-17 and true <= 1e-13
+
+
 # (g) -------------------------------------------------------------------------
 @pytest.mark.slow
 def test_paper_514_iterations(oracle_mod):
