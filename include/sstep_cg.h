@@ -109,6 +109,11 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  the Gram sums changes.  Auto: n >= 2^23 rows (the gathered vector cannot live in L2) and more than a
  *                  quarter of the entries further than 2^20 rows from the diagonal (e.g. config 5's randomly permuted
  *                  rows, where every 8-byte gather otherwise costs a 64-byte DRAM access).
+ *   "replace_every" 0 never (default, Alg. 3 as printed) | R > 0: residual replacement: after the block update
+ *                  of every R-th outer iteration -- unless the recurrence residual has just passed the stop test -- r is
+ *                  overwritten by the true residual b - A x (one extra SpMV + one pass), R_1 = D^-1 r and ||r||^2 follow,
+ *                  the directions P, AP are kept and the stop test is taken again.  Gram form only; such solves run on
+ *                  the graph path; b must stay valid until solve_end.
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);

@@ -40,13 +40,14 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
     const int* rp = nullptr;
     const int* ci = nullptr;
     const double* va = nullptr;
+    const double* b_cur = nullptr;  // right-hand side of the solve in progress (solver's numbering), for residual replacement
     bool ready = false, in_solve = false;
     // owned device memory
     double *dinv = nullptr, *R = nullptr, *AR = nullptr, *P = nullptr, *AP = nullptr, *x = nullptr, *r = nullptr;
@@ -473,6 +474,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "form" && (value == 0 || value == 1)) h->form = (int)value;
     else if (k == "resident" && value >= 0 && value <= 2) h->resident_opt = (int)value;
     else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
+    else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -493,6 +495,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "kernels_per_outer") *value = kernels_per_outer(h);
     else if (k == "basis") *value = h->basis;
     else if (k == "launches") *value = h->launches;
+    else if (k == "replace_every") *value = h->replace_every;
     else if (k == "reordered") *value = h->reordered ? 1 : 0;
     else if (k == "cm_levels") *value = h->cm_levels;
     else if (k == "cm_components") *value = h->cm_comps;
@@ -513,6 +516,8 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         return fail(h, SSTEP_CG_ERR_ARG, "setup: need n > 0, 0 < nnz < 2^31, non-null CSR arrays, 1 <= s <= 16");
     if (h->form == 1 && h->basis != SSTEP_CG_BASIS_MONOMIAL)
         return fail(h, SSTEP_CG_ERR_ARG, "setup: the moment form (Alg. 5 + Alg. 6) assumes the monomial basis");
+    if (h->form == 1 && h->replace_every > 0)
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: residual replacement needs the Gram form (Alg. 6 assumes r = r_prev - AP alpha)");
     CK(cudaSetDevice(h->device));
     CK(cudaStreamSynchronize(h->stream));
     free_problem(h);
@@ -639,7 +644,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     h->resident = false;
     h->res_grid = 0;
     // (auto: s <= 4 only -- above, the redundant per-CTA reduction of the 2s^2+s partials outweighs the saved launches)
-    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && n + 4096 < (int64_t(1) << 31)) {
+    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && h->replace_every == 0 && n + 4096 < (int64_t(1) << 31)) {
         int coop = 0;
         CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
         int64_t g = (n + 31) / 32;
@@ -664,7 +669,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     }
     if (h->resident_opt == 2 && !h->resident) {
         free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: resident path forced but the problem does not fit shared memory (or form = 1)");
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: resident path forced but the problem does not fit shared memory (or form = 1 / replace_every > 0)");
     }
 
     // workspaces
@@ -728,6 +733,7 @@ int sstep_cg_solve_begin(sstep_cg_t* h, const double* b, const double* x0, doubl
         }
         CK(cudaGetLastError());
     }
+    h->b_cur = b;
     if (x0) {  // r <- A x0 with the production SpMV, then r <- b - r in init_kernel
         CK(launch_spmv(h, sm, x0, h->r, nullptr, nullptr, 0, nullptr));
     }
@@ -757,6 +763,14 @@ int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
             CK(launch_outer(h, h->stream));
         }
         h->graph_launches++;
+        if (h->replace_every > 0 && h->graph_launches % h->replace_every == 0) {
+            // residual replacement: y = A x into AR(:,1) (scratch until the next MPK), r <- b - y, R_1, rho, stop test;
+            // both kernels exit at once if the update has just declared convergence or a breakdown
+            CK(launch_spmv(h, h->stream, h->x, h->AR, nullptr, nullptr, 0, h->st));
+            replace_kernel<<<h->init_grid, 256, 0, h->stream>>>(h->n, h->b_cur, h->AR, h->r, h->R, h->dinv, h->partials, h->st);
+            CK(cudaGetLastError());
+            h->launches++;
+        }
     }
     return 0;
 }

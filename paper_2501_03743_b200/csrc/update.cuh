@@ -95,7 +95,8 @@ __device__ __forceinline__ double update_half(int64_t n, int64_t row, const doub
 // (Alg. 3 l.31-33).  partials: [2][gridDim.x].  Every thread of the CTA calls.  MOM: only the moment form pays for mu^0.
 template <bool MOM>
 __device__ __forceinline__ void update_block_finish(double rho, double mu0, int nw, double* __restrict__ partials,
-                                                    ScgState* __restrict__ st, double* __restrict__ rho_out) {
+                                                    ScgState* __restrict__ st, double* __restrict__ rho_out,
+                                                    bool count_iteration = true) {
     __shared__ double red[MOM ? 2 : 1][32];
     __shared__ bool is_last;
     rho = warp_sum(rho);
@@ -124,7 +125,7 @@ __device__ __forceinline__ void update_block_finish(double rho, double mu0, int 
         if (threadIdx.x == 0) {
             st->rho = v;
             if (MOM) st->mu0 = w;
-            st->k = st->k + 1;
+            if (count_iteration) st->k = st->k + 1;
             if (rho_out) rho_out[0] = v;
             if (!isfinite(v)) st->status = 2;
             else if (sqrt(v) < st->rtol * sqrt(st->rho0)) st->status = 0;
@@ -160,6 +161,24 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
         if (MOM) mu0 = fma(r1, ri, mu0);  // moment form: mu^0 = R_1^T r
     }
     update_block_finish<MOM>(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
+}
+
+// ---- residual replacement (option "replace_every", reading A22): r <- b - A x with y = A x from the
+// production SpMV, R(:,1) <- D^-1 r, rho = ||r||^2 and the stop test taken again on the replaced residual.  P, AP stay.
+__global__ void __launch_bounds__(256)
+replace_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ y, double* __restrict__ r,
+               double* __restrict__ R1, const double* __restrict__ dinv, double* __restrict__ partials,
+               ScgState* __restrict__ st) {
+    if (st->status != SCG_RUNNING) return;
+    double rho = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        const double ri = b[row] - y[row];
+        r[row] = ri;
+        R1[row] = dinv[row] * ri;
+        rho = fma(ri, ri, rho);
+    }
+    update_block_finish<false>(rho, 0.0, (int)(blockDim.x >> 5), partials, st, nullptr, /*count_iteration=*/false);
 }
 
 // ---- start of a solve: r = b - A x0 (Ax0 already in r if have_ax), x = x0, R(:,1) = D^-1 r, rho0 = ||r||^2 ----

@@ -227,3 +227,38 @@ def test_solve_host_end_to_end(oracle_mod, cg_mod, torch_mod):
         x, res = h.solve_host(th(c["rowptr"]), th(c["colidx"]), th(c["vals"]), th(c["b"]), 2, rtol=1e-8, maxit=500)
     assert res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
     assert rel(x.numpy(), ref["x"]) <= 1e-8
+
+
+@pytest.mark.parametrize("cfg,N,s,R", [(2, 20, 3, 2), (1, 24, 2, 1), (5, 16, 4, 3), (3, 12, 4, 2)])
+def test_residual_replacement_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg, N, s, R):
+    """Option replace_every (reading A22) against the oracle's orc_sstep_rr: iterates, reported residuals
+    (the replaced, i.e. true, residual on every R-th iteration) and the full solve."""
+    c = gen.make_config(cfg, N=N, s=s)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    K = 6
+    ref = oracle_mod.sstep(rp, ci, v, b, s, rtol=0.0, maxit=K, xhist_cap=K, history=True, replace_every=R)
+    full = oracle_mod.sstep(rp, ci, v, b, s, rtol=c["rtol"], maxit=c["maxit"], replace_every=R)
+    with cg_mod.SStepCG(0, replace_every=R) as h:
+        h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), s)
+        assert h.get_info("resident") == 0 and h.get_info("replace_every") == R
+        bd = dev(torch_mod, b)
+        for k in range(1, K + 1):
+            h.solve_begin(bd, None, 0.0)
+            h.iterate(k)
+            x, res = h.solve_end()
+            assert res["outer_iters"] == k and res["status"] == 1
+            assert res["kernel_launches"] == 1 + k * (s + 2) + 2 * (k // R)
+            assert rel(x.cpu().numpy(), ref["xhist"][k - 1]) <= 1e-11
+            # (an iterate difference of 1e-11 moves a residual by up to ||A|| ||dx|| / ||b||: absolute floor 1e-13)
+            assert abs(res["relres"] - ref["hist"][k - 1]) <= 1e-9 * ref["hist"][k - 1] + 1e-13
+            if k % R == 0:     # the reported residual is the true one (oracle's SpMV of the GPU's iterate)
+                true = np.linalg.norm(b - oracle_mod.spmv(rp, ci, v, x.cpu().numpy())) / np.linalg.norm(b)
+                # (b - A x cancels: its rounding error is ~1e-16 (||b|| + ||A|| ||x||), an absolute floor on the residual norm)
+                assert abs(res["relres"] - true) <= 1e-12 * true + 1e-14
+        x, res = h.solve(bd, rtol=c["rtol"], maxit=c["maxit"])
+        assert full["status"] == 0 and res["status"] == 0 and abs(res["outer_iters"] - full["iters"]) <= 1
+        if res["outer_iters"] == full["iters"]:
+            assert rel(x.cpu().numpy(), full["x"]) <= 1e-8
+    with cg_mod.SStepCG(0, replace_every=2, form=1) as h:          # Alg. 6 assumes r = r_prev - AP alpha
+        with pytest.raises(cg_mod.SStepCGError, match="Gram form"):
+            h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), s)
