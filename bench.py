@@ -264,6 +264,25 @@ def run_ours(args):
             sweep[str(s)] = entry
             if s == s0:
                 primary = dict(entry, launches=launches, agg=agg, mb=mb)
+    # the textbook PCG of Alg. 1 as its own kernel sequence (option method = 1): the classical
+    # two-reduction comparator on the same workload; one "outer iteration" = one CG iteration
+    pcg = None
+    if args.pcg:
+        with cg.SStepCG(local, method=1) as h:
+            h.setup(rp, ci, va, 1)
+            ms, launches, res = time_outer_iterations(torch, h, b, 1, args.steps, args.warmup, barrier)
+            agg = aggregate_replicas(ms, args.steps, world, reduce_max)
+            us = 1e3 * agg["ms_per_step"]
+            bytes_it = 12 * nnz + 4 * (n + 1) + 8 * n * 12      # CSR + p, s | p, s, x, r -> x, r, u | u, p -> p
+            h.solve_begin(b, None, 0.0)
+            h.iterate(3)
+            t_spmv, t_upd, t_dir = h.profile_outer(10)
+            h.solve_end(want_x=False)
+            pcg = dict(us_per_iteration=us, model_gb_per_iteration=bytes_it / 1e9, achieved_gbs=bytes_it / (us * 1e-6) / 1e9,
+                       frac_of_measured_peak=bytes_it / (us * 1e-6) / 1e9 / peak, gdof_iter_per_s=world * n / (us * 1e-6) / 1e9,
+                       kernel_us=dict(spmv=1e2 * t_spmv, update=1e2 * t_upd, direction=1e2 * t_dir), launches=launches,
+                       note="Alg. 1 PCG-HS (PAPER.md:48-73), 3 kernels and 2 reductions per iteration; compare with "
+                            "us_per_cg_equiv_iter of the s-step entries")
     # resident path: what sstep_cg_solve runs by default when every CTA's rows fit shared memory
     resident = None
     with cg.SStepCG(local) as h:
@@ -276,7 +295,7 @@ def run_ours(args):
                             gdof_iter_per_s=world * n * s0 / (1e3 * agg["ms_per_step"] * 1e-6) / 1e9, relres_at_end=res["relres"],
                             note="whole loop in one cooperative launch per restart (csrc/resident.cuh); s + 1 grid barriers per outer iteration")
     return dict(world=world, rank=rank, local=local, c=c, n=n, nnz=nnz, N=N, sweep=sweep, moment=moment, primary=primary, clocks=clocks,
-                resident=resident,
+                resident=resident, pcg=pcg,
                 peak=peak, peak_src=peak_src, t_gen=t_gen, dev=(rp, ci, va, b))
 
 
@@ -295,7 +314,7 @@ def run_e2e(args, ctx):
     x = torch.empty(c["n"], dtype=torch.float64).pin_memory()
     best = None
     with cg.SStepCG(ctx["local"]) as h:
-        for _ in range(2):  # first pass warms allocator / graph instantiation paths; report the second
+        for it in range(3):  # first pass warms allocator / graph instantiation paths; report the faster of the next two
             ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
@@ -304,7 +323,9 @@ def run_e2e(args, ctx):
             ev1.record()
             torch.cuda.synchronize()
             wall_ms = 1e3 * (time.perf_counter() - t0)
-            best = dict(ms=max(ev0.elapsed_time(ev1), wall_ms), res=res)
+            cur = dict(ms=max(ev0.elapsed_time(ev1), wall_ms), res=res)
+            if it >= 1 and (best is None or cur["ms"] < best["ms"]):
+                best = cur
     k = best["res"]["outer_iters"]
     assert k >= 1 and best["res"]["status"] in (0, 1, 2), best
     xerr = None
@@ -408,6 +429,7 @@ def main():
     ap.add_argument("--sweep", type=str, default="1,2,4,8", help="block sizes also reported (config 4's sweep); '' = none")
     ap.add_argument("--no-moment-form", dest="moment_form", action="store_false",
                     help="skip the extra lines for the moment form (option form = 1) of the same block sizes")
+    ap.add_argument("--no-pcg", dest="pcg", action="store_false", help="skip the Alg. 1 (PCG-HS) comparator line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -474,6 +496,7 @@ def main():
         "kernels": {"us": p["kernel_us"], "gbs": p["kernel_gbs"], "frac_of_measured_peak": p["kernel_frac_of_measured_peak"],
                     "share_of_step": p["kernel_share_of_step"]},
         "sweep": ctx["sweep"],
+        "pcg_hs": ctx["pcg"],             # Alg. 1 as its own kernel sequence (comparator, not the headline)
         "resident_path": ctx["resident"],  # only for problems that fit shared memory (config 1), else null
         "moment_form": ctx["moment"],     # same solver with Alg. 5 + Alg. 6 (no Gram pass); not the headline
         "clocks": ctx["clocks"],

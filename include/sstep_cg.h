@@ -114,6 +114,11 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  overwritten by the true residual b - A x (one extra SpMV + one pass), R_1 = D^-1 r and ||r||^2 follow,
  *                  the directions P, AP are kept and the stop test is taken again.  Gram form only; such solves run on
  *                  the graph path; b must stay valid until solve_end.
+ *   "method"       0 (default) the s-step PCG of Alg. 3 | 1 the textbook PCG of Alg. 1 (PCG-HS) as its own
+ *                  kernel sequence (SpMV with the p^T A p partials, fused x / r / u update with both reductions and the
+ *                  stop test, direction update): the classical two-reduction comparator.  Needs s = 1 at setup;
+ *                  "outer iterations" are then CG iterations.  (The paper's one-reduction baseline "fcg", Alg. 2, is
+ *                  method 0 with s = 1.)
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);

@@ -1,0 +1,86 @@
+// pcg.cuh -- SURVEY.md 8(f) NEXT-3: the textbook preconditioned CG of Alg. 1 (PCG-HS) as its own kernel
+// sequence (option "method" = 1), the classical comparator with TWO reductions per iteration:
+//   K1  s_k = A p_k, with the per-block partials of p_k^T s_k in the SpMV epilogue        (spmv.cuh, moment epilogue)
+//   K2  alpha_k = u_k^T r_k / p_k^T s_k ; x += alpha p ; r -= alpha s ; u = D^-1 r ; partials of u^T r and r^T r ;
+//       cross-block finish: beta_k = u_{k+1}^T r_{k+1} / u_k^T r_k, k <- k + 1, stop test ||r|| < rtol ||r_0||
+//   K3  p = u + beta_k p
+// Workspaces of the s-step path at s = 1 are reused: p = P, s = AP, u = R(:,1); u^T r lives in ScgState::mu0,
+// alpha / beta in ScgState::alpha[0] / beta[0].  HBM bytes per iteration: CSR + 8n (2 + 7 + 3).
+#pragma once
+#include "common.cuh"
+#include "update.cuh"
+
+// K2.  ps_partials: [nps] per-block partials of p^T s left by the SpMV (summed here by EVERY block in the same fixed
+// order, so all blocks use the same alpha).  partials: [2][gridDim.x] scratch for u^T r and r^T r.
+__global__ void __launch_bounds__(256, 4)
+pcg_update_kernel(int64_t n, const double* __restrict__ p, const double* __restrict__ sk, double* __restrict__ x,
+                  double* __restrict__ r, double* __restrict__ u, const double* __restrict__ dinv,
+                  const double* __restrict__ ps_partials, int nps, double* __restrict__ partials, ScgState* __restrict__ st) {
+    if (st->status != SCG_RUNNING) return;
+    __shared__ double s_alpha;
+    __shared__ double red[2][8];
+    __shared__ bool is_last;
+    if (threadIdx.x < 32) {
+        const double ps = warp_sum_array(ps_partials, nps, (int)threadIdx.x);
+        if (threadIdx.x == 0) s_alpha = (ps > 0.0 && isfinite(ps)) ? st->mu0 / ps : nan("");
+    }
+    __syncthreads();
+    const double alpha = s_alpha;
+    if (!isfinite(alpha)) {  // p^T A p <= 0 or not finite: breakdown, x keeps the last iterate (every block decides alike)
+        if (blockIdx.x == 0 && threadIdx.x == 0) st->status = 2;
+        return;
+    }
+    double ur = 0.0, rr = 0.0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
+        const double pi = ldg_stream(p + row), si = ldg_stream(sk + row);
+        const double xi = fma(alpha, pi, x[row]);
+        const double ri = fma(-alpha, si, r[row]);
+        const double ui = dinv[row] * ri;
+        x[row] = xi;
+        r[row] = ri;
+        u[row] = ui;
+        ur = fma(ui, ri, ur);
+        rr = fma(ri, ri, rr);
+    }
+    ur = warp_sum(ur);
+    rr = warp_sum(rr);
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = ur; red[1][threadIdx.x >> 5] = rr; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { a += red[0][w]; b += red[1][w]; }
+        partials[blockIdx.x] = a;
+        partials[gridDim.x + blockIdx.x] = b;
+        __threadfence();
+        const unsigned int t = atomicAdd(&st->ticket_update, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    if (threadIdx.x < 32) {
+        __threadfence();
+        const double a = warp_sum_array(partials, (int)gridDim.x, (int)threadIdx.x);
+        const double b = warp_sum_array(partials + gridDim.x, (int)gridDim.x, (int)threadIdx.x);
+        if (threadIdx.x == 0) {
+            st->alpha[0] = alpha;
+            st->beta[0] = a / st->mu0;  // beta_k = u_{k+1}^T r_{k+1} / u_k^T r_k
+            st->mu0 = a;
+            st->rho = b;
+            st->k = st->k + 1;
+            if (!isfinite(b) || !isfinite(a)) st->status = 2;
+            else if (sqrt(b) < st->rtol * sqrt(st->rho0)) st->status = 0;
+            st->ticket_update = 0;
+        }
+    }
+}
+
+// K3: p = u + beta p
+__global__ void __launch_bounds__(256, 4)
+pcg_direction_kernel(int64_t n, const double* __restrict__ u, double* __restrict__ p, const ScgState* __restrict__ st) {
+    if (st->status != SCG_RUNNING) return;
+    const double beta = st->beta[0];
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride)
+        p[row] = fma(beta, p[row], ldg_stream(u + row));
+}

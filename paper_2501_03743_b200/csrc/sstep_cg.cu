@@ -11,6 +11,7 @@
 #include "gram.cuh"
 #include "gram_tma.cuh"
 #include "moment.cuh"
+#include "pcg.cuh"
 #include "reorder.cuh"
 #include "resident.cuh"
 #include "spmv.cuh"
@@ -40,7 +41,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -159,7 +160,7 @@ cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
     if (h->bulk) {
-        auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0, h->bulk_cap);
+        auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0 || h->method == 1, h->bulk_cap);
         const size_t smem = bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc);
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -356,8 +357,24 @@ cudaError_t launch_sw(sstep_cg* h, cudaStream_t sm, ScgState* st, int do_solve) 
     return cudaGetLastError();
 }
 
+// one iteration of Alg. 1 (method = 1; pcg.cuh): p = P, s_k = AP, u = R
+cudaError_t launch_pcg_iteration(sstep_cg* h, cudaStream_t sm, cudaEvent_t* evs = nullptr) {
+    if (evs) cudaEventRecord(evs[0], sm);
+    cudaError_t e = launch_spmv(h, sm, h->P, h->AP, nullptr, nullptr, 0, h->st, h->mom, nullptr);
+    if (e != cudaSuccess) return e;
+    if (evs) { cudaEventRecord(evs[1], sm); cudaEventRecord(evs[2], sm); }
+    pcg_update_kernel<<<h->update_grid_reg, 256, 0, sm>>>(h->n, h->P, h->AP, h->x, h->r, h->R, h->dinv, h->mom, h->spmv_grid,
+                                                         h->partials, h->st);
+    if (evs) { cudaEventRecord(evs[3], sm); cudaEventRecord(evs[4], sm); }
+    pcg_direction_kernel<<<h->update_grid_reg, 256, 0, sm>>>(h->n, h->R, h->P, h->st);
+    if (evs) cudaEventRecord(evs[5], sm);
+    h->launches += 2;
+    return cudaGetLastError();
+}
+
 // one outer iteration on the production buffers (Alg. 3 l.5-21)
 cudaError_t launch_outer(sstep_cg* h, cudaStream_t sm) {
+    if (h->method == 1) return launch_pcg_iteration(h, sm);
     cudaError_t e = launch_mpk(h, sm, h->R, h->AR, h->st);
     if (e != cudaSuccess) return e;
     e = h->form ? launch_sw(h, sm, h->st, 1) : launch_gram(h, sm, false, h->R, h->AR, h->AP, h->r, h->st, 1);
@@ -400,7 +417,7 @@ void free_owned(sstep_cg* h) {
     h->own_va = h->own_b = h->own_x = nullptr;
 }
 
-int kernels_per_outer(const sstep_cg* h) { return h->s + 2; }
+int kernels_per_outer(const sstep_cg* h) { return h->method == 1 ? 3 : h->s + 2; }
 
 __global__ void iota_kernel(int64_t n, int* __restrict__ p) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -475,6 +492,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "resident" && value >= 0 && value <= 2) h->resident_opt = (int)value;
     else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
     else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
+    else if (k == "method" && (value == 0 || value == 1)) h->method = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -496,6 +514,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "basis") *value = h->basis;
     else if (k == "launches") *value = h->launches;
     else if (k == "replace_every") *value = h->replace_every;
+    else if (k == "method") *value = h->method;
     else if (k == "reordered") *value = h->reordered ? 1 : 0;
     else if (k == "cm_levels") *value = h->cm_levels;
     else if (k == "cm_components") *value = h->cm_comps;
@@ -516,6 +535,8 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         return fail(h, SSTEP_CG_ERR_ARG, "setup: need n > 0, 0 < nnz < 2^31, non-null CSR arrays, 1 <= s <= 16");
     if (h->form == 1 && h->basis != SSTEP_CG_BASIS_MONOMIAL)
         return fail(h, SSTEP_CG_ERR_ARG, "setup: the moment form (Alg. 5 + Alg. 6) assumes the monomial basis");
+    if (h->method == 1 && (s != 1 || h->form != 0 || h->basis != 0 || h->replace_every > 0))
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: method = 1 (Alg. 1 PCG) takes s = 1 and none of form / basis / replace_every");
     if (h->form == 1 && h->replace_every > 0)
         return fail(h, SSTEP_CG_ERR_ARG, "setup: residual replacement needs the Gram form (Alg. 6 assumes r = r_prev - AP alpha)");
     CK(cudaSetDevice(h->device));
@@ -644,7 +665,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     h->resident = false;
     h->res_grid = 0;
     // (auto: s <= 4 only -- above, the redundant per-CTA reduction of the 2s^2+s partials outweighs the saved launches)
-    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && h->replace_every == 0 && n + 4096 < (int64_t(1) << 31)) {
+    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && h->replace_every == 0 && h->method == 0 && n + 4096 < (int64_t(1) << 31)) {
         int coop = 0;
         CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
         int64_t g = (n + 31) / 32;
@@ -740,6 +761,7 @@ int sstep_cg_solve_begin(sstep_cg_t* h, const double* b, const double* x0, doubl
     init_kernel<<<h->init_grid, 256, 0, sm>>>(h->n, b, x0, x0 ? 1 : 0, h->x, h->r, h->R, h->dinv, h->partials, h->st, h->s, rtol);
     h->launches++;
     CK(cudaGetLastError());
+    if (h->method == 1) CK(cudaMemcpyAsync(h->P, h->R, sizeof(double) * h->n, cudaMemcpyDeviceToDevice, sm));  // p_0 = u_0 (Alg. 1 l.3)
     h->in_solve = true;
     return 0;
 }
@@ -780,6 +802,23 @@ int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "profile_outer: call solve_begin first");
     if (h->resident) return fail(h, SSTEP_CG_ERR_STATE, "profile_outer: the resident path has no per-kernel launches (set option resident = 1)");
     cudaStream_t sm = h->stream;
+    if (h->method == 1) {  // Alg. 1: ms_host[0] = SpMV, [1] = update (K2), [2] = direction (K3)
+        cudaEvent_t ev[6];
+        for (auto& e : ev) CK(cudaEventCreate(&e));
+        ms_host[0] = ms_host[1] = ms_host[2] = 0.0;
+        int rc1 = 0;
+        for (int rep = 0; rep < reps && rc1 == 0; rep++) {
+            if (launch_pcg_iteration(h, sm, ev) != cudaSuccess || cudaStreamSynchronize(sm) != cudaSuccess) { rc1 = SSTEP_CG_ERR_CUDA; break; }
+            h->graph_launches++;
+            for (int k = 0; k < 3; k++) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, ev[2 * k], ev[2 * k + 1]);
+                ms_host[k] += ms;
+            }
+        }
+        for (auto& e : ev) cudaEventDestroy(e);
+        return rc1 ? fail(h, rc1, "profile_outer: CUDA error in the PCG iteration") : 0;
+    }
     const int per = h->s + 2;
     const int nev = reps * per * 2;
     cudaEvent_t* evs = new cudaEvent_t[nev];

@@ -262,3 +262,45 @@ def test_residual_replacement_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg,
     with cg_mod.SStepCG(0, replace_every=2, form=1) as h:          # Alg. 6 assumes r = r_prev - AP alpha
         with pytest.raises(cg_mod.SStepCGError, match="Gram form"):
             h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), s)
+
+
+@pytest.mark.parametrize("cfg,N", [(1, 24), (2, 20), (3, 12), (5, 14)])
+def test_pcg_method_matches_oracle_alg1(oracle_mod, cg_mod, torch_mod, cfg, N):
+    """Option method = 1: the textbook PCG (Alg. 1) as its own kernel sequence against the oracle's
+    orc_pcg: iterates, residual history, iteration count, final solution; graph and direct launches agree bitwise."""
+    c = gen.make_config(cfg, N=N)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    K = 8
+    ref = oracle_mod.pcg(rp, ci, v, b, rtol=0.0, maxit=K, xhist_cap=K, history=True)
+    full = oracle_mod.pcg(rp, ci, v, b, rtol=c["rtol"], maxit=5000)
+    xs = []
+    for use_graph in (1, 0):
+        with cg_mod.SStepCG(0, method=1, use_graph=use_graph) as h:
+            h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), 1)
+            assert h.get_info("kernels_per_outer") == 3 and h.get_info("resident") == 0
+            bd = dev(torch_mod, b)
+            for k in (1, 2, 5, K):
+                h.solve_begin(bd, None, 0.0)
+                h.iterate(k)
+                x, res = h.solve_end()
+                assert res["outer_iters"] == k and res["status"] == 1 and res["kernel_launches"] == 1 + 3 * k
+                assert rel(x.cpu().numpy(), ref["xhist"][k - 1]) <= 1e-12
+                assert abs(res["relres"] - ref["hist"][k - 1]) <= 1e-10 * ref["hist"][k - 1]
+            x, res = h.solve(bd, rtol=c["rtol"], maxit=5000)
+            assert full["status"] == 0 and res["status"] == 0 and abs(res["outer_iters"] - full["iters"]) <= 1
+            if res["outer_iters"] == full["iters"]:
+                assert rel(x.cpu().numpy(), full["x"]) <= 1e-8
+            xs.append(x.cpu().numpy())
+            # x0 != 0 and per-kernel times through profile_outer
+            x0 = np.random.default_rng(3).uniform(-1, 1, c["n"])
+            r0 = oracle_mod.pcg(rp, ci, v, b, x0=x0, rtol=c["rtol"], maxit=5000)
+            x, res = h.solve(bd, dev(torch_mod, x0), rtol=c["rtol"], maxit=5000)
+            assert res["status"] == 0 and abs(res["outer_iters"] - r0["iters"]) <= 1
+            h.solve_begin(bd, None, 0.0)
+            t = h.profile_outer(2)
+            _, res = h.solve_end(want_x=False)
+            assert res["outer_iters"] == 2 and all(ms > 0 for ms in t)
+    assert np.array_equal(xs[0], xs[1])
+    with cg_mod.SStepCG(0, method=1) as h:
+        with pytest.raises(cg_mod.SStepCGError, match="s = 1"):
+            h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), 2)
