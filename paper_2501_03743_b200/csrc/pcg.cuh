@@ -32,14 +32,42 @@ pcg_update_kernel(int64_t n, const double* __restrict__ p, const double* __restr
     }
     double ur = 0.0, rr = 0.0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
-        const double pi = ldg_stream(p + row), si = ldg_stream(sk + row);
-        const double xi = fma(alpha, pi, x[row]);
-        const double ri = fma(-alpha, si, r[row]);
+    // two rows per thread as 128-bit vectors (all operands are cudaMalloc'ed workspaces: 16-byte aligned); odd tail below
+    const int64_t n2 = n >> 1;
+    const double2* p2 = reinterpret_cast<const double2*>(p);
+    const double2* s2 = reinterpret_cast<const double2*>(sk);
+    const double2* d2 = reinterpret_cast<const double2*>(dinv);
+    double2* x2 = reinterpret_cast<double2*>(x);
+    double2* r2 = reinterpret_cast<double2*>(r);
+    double2* u2 = reinterpret_cast<double2*>(u);
+    auto one = [&](double2 pi, double2 si, double2 di, double2 xi, double2 ri, int64_t i) {
+        double2 ui;
+        xi.x = fma(alpha, pi.x, xi.x); xi.y = fma(alpha, pi.y, xi.y);
+        ri.x = fma(-alpha, si.x, ri.x); ri.y = fma(-alpha, si.y, ri.y);
+        ui.x = di.x * ri.x; ui.y = di.y * ri.y;
+        x2[i] = xi; r2[i] = ri; u2[i] = ui;
+        ur = fma(ui.x, ri.x, ur); ur = fma(ui.y, ri.y, ur);
+        rr = fma(ri.x, ri.x, rr); rr = fma(ri.y, ri.y, rr);
+    };
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + stride < n2; i += 2 * stride) {  // two independent row pairs per trip: ten 128-bit loads in flight
+        const int64_t j = i + stride;
+        const double2 pa = ldg_stream2(reinterpret_cast<const double*>(p2 + i)), pb = ldg_stream2(reinterpret_cast<const double*>(p2 + j));
+        const double2 sa = ldg_stream2(reinterpret_cast<const double*>(s2 + i)), sb = ldg_stream2(reinterpret_cast<const double*>(s2 + j));
+        const double2 da = d2[i], db = d2[j];
+        const double2 xa = x2[i], xb = x2[j];
+        const double2 ra = r2[i], rb = r2[j];
+        one(pa, sa, da, xa, ra, i);
+        one(pb, sb, db, xb, rb, j);
+    }
+    if (i < n2)
+        one(ldg_stream2(reinterpret_cast<const double*>(p2 + i)), ldg_stream2(reinterpret_cast<const double*>(s2 + i)), d2[i], x2[i], r2[i], i);
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int64_t row = n - 1;
+        const double xi = fma(alpha, p[row], x[row]);
+        const double ri = fma(-alpha, sk[row], r[row]);
         const double ui = dinv[row] * ri;
-        x[row] = xi;
-        r[row] = ri;
-        u[row] = ui;
+        x[row] = xi; r[row] = ri; u[row] = ui;
         ur = fma(ui, ri, ur);
         rr = fma(ri, ri, rr);
     }
@@ -81,6 +109,14 @@ pcg_direction_kernel(int64_t n, const double* __restrict__ u, double* __restrict
     if (st->status != SCG_RUNNING) return;
     const double beta = st->beta[0];
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride)
-        p[row] = fma(beta, p[row], ldg_stream(u + row));
+    const int64_t n2 = n >> 1;
+    double2* p2 = reinterpret_cast<double2*>(p);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += stride) {
+        const double2 ui = ldg_stream2(u + 2 * i);
+        double2 pi = p2[i];
+        pi.x = fma(beta, pi.x, ui.x);
+        pi.y = fma(beta, pi.y, ui.y);
+        p2[i] = pi;
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) p[n - 1] = fma(beta, p[n - 1], u[n - 1]);
 }

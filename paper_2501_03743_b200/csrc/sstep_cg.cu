@@ -64,7 +64,7 @@ struct sstep_cg {
     int lanes = 1;
     bool bulk = false;
     int bulk_cap = 256, bulk_wpc = 8;
-    int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0;
+    int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0, pcg_grid = 0;
     bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int64_t num_tiles = 0;
@@ -363,10 +363,10 @@ cudaError_t launch_pcg_iteration(sstep_cg* h, cudaStream_t sm, cudaEvent_t* evs 
     cudaError_t e = launch_spmv(h, sm, h->P, h->AP, nullptr, nullptr, 0, h->st, h->mom, nullptr);
     if (e != cudaSuccess) return e;
     if (evs) { cudaEventRecord(evs[1], sm); cudaEventRecord(evs[2], sm); }
-    pcg_update_kernel<<<h->update_grid_reg, 256, 0, sm>>>(h->n, h->P, h->AP, h->x, h->r, h->R, h->dinv, h->mom, h->spmv_grid,
+    pcg_update_kernel<<<h->pcg_grid, 256, 0, sm>>>(h->n, h->P, h->AP, h->x, h->r, h->R, h->dinv, h->mom, h->spmv_grid,
                                                          h->partials, h->st);
     if (evs) { cudaEventRecord(evs[3], sm); cudaEventRecord(evs[4], sm); }
-    pcg_direction_kernel<<<h->update_grid_reg, 256, 0, sm>>>(h->n, h->R, h->P, h->st);
+    pcg_direction_kernel<<<h->pcg_grid, 256, 0, sm>>>(h->n, h->R, h->P, h->st);
     if (evs) cudaEventRecord(evs[5], sm);
     h->launches += 2;
     return cudaGetLastError();
@@ -659,6 +659,10 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     {
         int64_t want = (n + 255) / 256, cap = (int64_t)h->num_sms * 8;
         h->init_grid = (int)(want < cap ? want : cap);
+        want = (n / 2 + 255) / 256;
+        if (want < 1) want = 1;
+        cap = (int64_t)h->num_sms * 4;  // Alg. 1 kernels: two rows per thread, 4 CTAs per SM
+        h->pcg_grid = (int)(want < cap ? want : cap);
     }
 
     // resident path: whole loop in one cooperative launch when every CTA's rows fit shared memory
@@ -704,6 +708,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     size_t np = (size_t)h->gram_grid * (2 * s * s + s);
     if (np < 2 * (size_t)h->update_grid) np = 2 * (size_t)h->update_grid;
     if (np < 2 * (size_t)h->init_grid) np = 2 * (size_t)h->init_grid;
+    if (np < 2 * (size_t)h->pcg_grid) np = 2 * (size_t)h->pcg_grid;
     if (np < (size_t)h->res_grid * (2 * s * s + s + 1)) np = (size_t)h->res_grid * (2 * s * s + s + 1);
     CK(cudaMalloc(&h->partials, sizeof(double) * np));
     CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
