@@ -676,13 +676,17 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         if (g > h->num_sms) g = h->num_sms;
         int64_t rpb = ((n + g - 1) / g + 31) / 32 * 32;
         g = (n + rpb - 1) / rpb;
-        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
-        tile_nnz_max_kernel<<<(unsigned)((g + 255) / 256), 256, 0, sm>>>(n, rowptr, (int)rpb, g, h->iscratch + 3);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
-        CK(cudaStreamSynchronize(sm));
+        // (the vectors alone must fit: skips the tile scan for every problem that is far too large)
+        if (resident_smem_bytes(s, (int)(rpb < (1 << 20) ? rpb : (1 << 20)), 0) > (size_t)200 * 1024) coop = 0;
+        if (coop) {
+            CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
+            tile_nnz_max_kernel<<<(unsigned)((g + 255) / 256), 256, 0, sm>>>(n, rowptr, (int)rpb, g, h->iscratch + 3);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+        }
         const int nzcap = (hs[3] + 3) & ~3;
-        const size_t bytes = resident_smem_bytes(s, (int)rpb, nzcap);
+        const size_t bytes = coop ? resident_smem_bytes(s, (int)rpb, nzcap) : 0;
         if (coop && bytes <= (size_t)200 * 1024) {
             h->res_grid = (int)g; h->res_rpb = (int)rpb; h->res_nzcap = nzcap; h->res_smem = bytes;
             h->res_threads = (int)(rpb < 512 ? rpb : 512);
