@@ -119,3 +119,37 @@ def test_fullsize_graph_replay_matches_oracle_iterates(cg_mod, torch_mod, full):
             assert res["outer_iters"] == k and res["status"] == 1
             xr = full["xs"][k - 1]
             assert np.linalg.norm(x.cpu().numpy() - xr) <= 1e-10 * np.linalg.norm(xr), k
+
+
+def test_config3_full_size(oracle_mod, cg_mod, torch_mod):
+    """BASELINE.json config 3 at full size (27-point 160^3, n = 4 096 000, nnz = 109 215 352, s = 4) in the launch
+    configuration bench.py times (bulk-staged SpMV, two lanes per row, 512-entry tiles): every row of one SpMV, the
+    first three iterates of the graph-replayed loop, and the full solve (x within 1e-8, outer iterations within +-1)."""
+    c = gen.make_config(3)
+    rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
+    n = c["n"]
+    assert n == 160 ** 3 and c["nnz"] == (3 * 160 - 2) ** 3
+    t = lambda a: dev(torch_mod, a)
+    ref = oracle_mod.sstep(rp, ci, v, b, 4, rtol=1e-8, maxit=2000, xhist_cap=3)
+    with cg_mod.SStepCG(0) as h:
+        h.setup(t(rp), t(ci), t(v), 4)
+        assert h.get_info("spmv_bulk") == 1 and h.get_info("lanes") == 2 and h.get_info("reordered") == 0
+        x = np.random.default_rng(13).uniform(-1, 1, n)
+        y, yj = h.test_spmv(t(x))
+        yo = oracle_mod.spmv(rp, ci, v, x)
+        scale = oracle_mod.spmv(rp, ci, np.abs(v), np.abs(x))
+        assert np.all(np.abs(y.cpu().numpy() - yo) <= TOL_ROW * scale)
+        assert np.all(np.abs(yj.cpu().numpy() - yo / 26.0) <= TOL_ROW * scale / 26.0)
+        del y, yj, yo, scale
+        bd = t(b)
+        for k in (1, 2, 3):
+            h.solve_begin(bd, None, 0.0)
+            h.iterate(k)
+            xk, res = h.solve_end()
+            assert res["outer_iters"] == k
+            assert np.linalg.norm(xk.cpu().numpy() - ref["xhist"][k - 1]) <= 1e-10 * np.linalg.norm(ref["xhist"][k - 1]), k
+        xg, res = h.solve(bd, rtol=1e-8, maxit=2000)
+        assert ref["status"] == 0 and res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
+        if res["outer_iters"] != ref["iters"]:
+            xg, _ = h.solve(bd, rtol=0.0, maxit=ref["iters"])
+        assert np.linalg.norm(xg.cpu().numpy() - ref["x"]) <= 1e-8 * np.linalg.norm(ref["x"])
