@@ -89,6 +89,17 @@ __global__ void first_unseen_kernel(int n, const int* __restrict__ level, int* _
     if (i < n && level[i] == -1) atomicMin(out, i);
 }
 
+// nodes not numbered yet (level == -1) keep their relative order and go to the end: flag -> exclusive scan -> place
+__global__ void flag_unseen_kernel(int n, const int* __restrict__ level, int* __restrict__ flag) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) flag[i] = (level[i] == -1) ? 1 : 0;
+}
+__global__ void place_unseen_kernel(int n, const int* __restrict__ level, const int* __restrict__ offs, int base,
+                                    int* __restrict__ perm, int* __restrict__ rank) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && level[i] == -1) { perm[base + offs[i]] = i; rank[i] = base + offs[i]; }
+}
+
 __global__ void set_root_kernel(int root, int pos, int* __restrict__ level, int* __restrict__ perm, int* __restrict__ rank) {
     level[root] = 0;
     if (perm) { perm[pos] = root; rank[root] = pos; }
@@ -139,8 +150,9 @@ inline int bits_for(unsigned int maxval) {
     } while (0)
 
 // Cuthill-McKee numbering of the graph of (rp, ci).  perm[new] = old, rank[old] = new (device, n ints each).
-// *done = false (and perm/rank undefined) if the graph has more than `max_components` components -- the caller then
-// keeps the original numbering.  levels_out / comps_out: statistics.
+// After `max_components` components (a matrix with very many tiny components would otherwise cost one BFS each) the
+// nodes still unnumbered are appended in their original order.  *done = false only on a CUDA error.
+// levels_out / comps_out: statistics (comps_out counts the components numbered by BFS).
 inline cudaError_t cuthill_mckee(int n, const int* rp, const int* ci, cudaStream_t sm, int* perm, int* rank, bool* done,
                                  int* levels_out, int* comps_out, int max_components = 64) {
     *done = false;
@@ -169,7 +181,24 @@ inline cudaError_t cuthill_mckee(int n, const int* rp, const int* ci, cudaStream
         const int vbits = bits_for((unsigned)(n - 1));
         int placed = 0, comps = 0, levels = 0, h = 0;
         while (placed < n) {
-            if (comps >= max_components) return cudaSuccess;  // *done stays false
+            if (comps >= max_components) {  // append the rest in index order
+                int* flag = reinterpret_cast<int*>(keys);
+                int* offs = reinterpret_cast<int*>(keys2);
+                flag_unseen_kernel<<<blocks_for(n), 256, 0, sm>>>(n, level, flag);
+                size_t tb = tmp_bytes;
+                size_t need = 0;
+                SCG_RCK(cub::DeviceScan::ExclusiveSum(nullptr, need, flag, offs, n, sm));
+                if (need > tb) {
+                    cudaFree(tmp);
+                    tmp = nullptr;
+                    SCG_RCK(cudaMalloc(&tmp, need));
+                    tmp_bytes = tb = need;
+                }
+                SCG_RCK(cub::DeviceScan::ExclusiveSum(tmp, tb, flag, offs, n, sm));
+                place_unseen_kernel<<<blocks_for(n), 256, 0, sm>>>(n, level, offs, placed, perm, rank);
+                placed = n;
+                break;
+            }
             // ---- a start node of this component: the smallest unnumbered index
             int start = 0;
             if (comps > 0) {

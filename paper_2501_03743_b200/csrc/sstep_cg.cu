@@ -602,7 +602,7 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
                 free_problem(h);
                 return fail(h, SSTEP_CG_ERR_CUDA, "setup: internal error, the permuted matrix failed validation");
             }
-        } else {  // too many connected components: keep the caller's numbering
+        } else {
             cudaFree(h->perm); cudaFree(h->rank);
             h->perm = h->rank = nullptr;
         }

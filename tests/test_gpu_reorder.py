@@ -142,15 +142,30 @@ def test_components_and_fallback(oracle_mod, cg_mod, torch_mod):
         check_cuthill_mckee(rp, ci, h.get_permutation().cpu().numpy().astype(np.int64))
         x, res = h.solve(t(b), rtol=1e-10, maxit=500)
     assert res["status"] == 0 and rel(x.cpu().numpy(), np.linalg.solve(A.toarray(), b)) <= 1e-8
-    # a diagonal matrix has n components: the numbering is abandoned, the caller's order kept (identity permutation)
+    # a diagonal matrix has n components: after 64 of them the rest is appended in index order (here: the identity)
     n = 200
     rp = np.arange(n + 1, dtype=np.int32); ci = np.arange(n, dtype=np.int32); v = np.linspace(1.0, 2.0, n)
     with cg_mod.SStepCG(0, reorder=2) as h:
         h.setup(t(rp), t(ci), t(v), 1)
-        assert h.get_info("reordered") == 0
+        assert h.get_info("reordered") == 1 and h.get_info("cm_components") == 64
         assert np.array_equal(h.get_permutation().cpu().numpy(), np.arange(n))
         x, res = h.solve(t(np.ones(n)), rtol=1e-12, maxit=5)
     assert res["status"] == 0 and np.allclose(x.cpu().numpy(), 1.0 / v, rtol=1e-12)
+    # a grid plus 100 isolated unknowns (scattered through the numbering): the grid is numbered by BFS, the isolated
+    # ones within the first 64 components or appended; the result is a valid permutation and the solve is right
+    rpg, cig, vg = gen.poisson7(7)
+    Ag = sp.csr_matrix((vg, cig, rpg))
+    A = sp.block_diag([sp.identity(60) * 3.0, Ag, sp.identity(40) * 5.0], format="csr")
+    prm = np.random.default_rng(2).permutation(A.shape[0])
+    A = A[prm][:, prm].tocsr(); A.sort_indices()
+    rp, ci, v = A.indptr.astype(np.int32), A.indices.astype(np.int32), A.data.astype(np.float64)
+    b = np.random.default_rng(9).uniform(-1, 1, A.shape[0])
+    with cg_mod.SStepCG(0, reorder=2) as h:
+        h.setup(t(rp), t(ci), t(v), 2)
+        perm = h.get_permutation().cpu().numpy()
+        assert h.get_info("reordered") == 1 and np.array_equal(np.sort(perm), np.arange(A.shape[0]))
+        x, res = h.solve(t(b), rtol=1e-10, maxit=500)
+    assert res["status"] == 0 and rel(x.cpu().numpy(), np.linalg.solve(A.toarray(), b)) <= 1e-8
     # auto never reorders small or already-local systems
     rp, ci, v = gen.poisson7(16)
     with cg_mod.SStepCG(0) as h:
