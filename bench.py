@@ -168,6 +168,7 @@ def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
     """CUDA-event time (ms) of exactly k_steps outer iterations (graph replays) on the solver's stream."""
     R = restart_every_for(s)
     resident = h.get_info("resident") == 1      # whole loop in one cooperative launch: init + 1 launch per restart
+    kpo = h.get_info("kernels_per_outer")
     h.solve_begin(b, None, 0.0)
     h.iterate(warmup)
     _, res = h.solve_end(want_x=False)
@@ -182,7 +183,7 @@ def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
         h.solve_begin(b, None, 0.0)
         h.iterate(k)
         done += k
-        launches += 2 if resident else 1 + k * (s + 2)
+        launches += 2 if resident else 1 + k * kpo
     ev1.record()
     torch.cuda.synchronize()
     barrier()

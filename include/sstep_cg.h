@@ -119,6 +119,15 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  stop test, direction update): the classical two-reduction comparator.  Needs s = 1 at setup;
  *                  "outer iterations" are then CG iterations.  (The paper's one-reduction baseline "fcg", Alg. 2, is
  *                  method 0 with s = 1.)
+ *   "mpk_fused"    0 / 1 off (default) | 2 on (EXPERIMENTAL).  Wavefront-ordered matrix-powers kernel (csrc/mpk_wave.cuh):
+ *                  the s SpMVs of Alg. 4 run as ONE kernel whose levels follow each other down a banded matrix a few row
+ *                  blocks apart, so that the CSR arrays (and the basis vectors) are re-read from L2 instead of HBM.
+ *                  Applies to thread-per-row matrices on the bulk-staged SpMV (7-point configs) with s >= 2, form = 0,
+ *                  n % 4 == 0; bitwise the same results as the separate SpMVs.  Measured on 320^3: DRAM reads per two
+ *                  levels 3.2 -> 1.6 GB as designed, but 820 us per level against 550 us (the statically assigned,
+ *                  in-order tiles couple every warp to the slowest one), hence not selected automatically.
+ *                  "mpk_block_rows" (32 * 2^k; 0 = auto), "mpk_levels" (levels per pass) and "mpk_slack" (extra blocks
+ *                  a level trails its predecessor by) override the shape.
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);

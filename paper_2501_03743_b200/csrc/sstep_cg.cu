@@ -11,6 +11,7 @@
 #include "gram.cuh"
 #include "gram_tma.cuh"
 #include "moment.cuh"
+#include "mpk_wave.cuh"
 #include "pcg.cuh"
 #include "reorder.cuh"
 #include "resident.cuh"
@@ -41,7 +42,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0, mpk_fused_opt = 0, mpk_block_opt = 0, mpk_levels_opt = 0, mpk_slack_opt = -1;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -75,6 +76,10 @@ struct sstep_cg {
     int *own_prp = nullptr, *own_pci = nullptr;
     double *own_pva = nullptr, *bperm = nullptr, *x0perm = nullptr;
     int cm_levels = 0, cm_comps = 0, far_permille = 0;
+    // wavefront-fused matrix-powers kernel (mpk_wave.cuh): the CSR arrays are read from HBM once per pass of `mw_levels` levels
+    bool mpk_fused = false;
+    int bandwidth = 0, mw_tpb = 0, mw_nb = 0, mw_lag = 0, mw_lag_dep = 0, mw_levels = 0;
+    int* mw_sync = nullptr;  // [s * nb] done counters, then [s] watermarks
     // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
     bool resident = false;
     int res_grid = 0, res_rpb = 0, res_nzcap = 0, res_threads = 0;
@@ -333,6 +338,24 @@ cudaError_t resident_op(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ
 // Alg. 4 on the given buffers: s Jacobi-fused SpMVs (R(:,1) must already hold D^-1 r)
 cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, const ScgState* st) {
     const int64_t n = h->n;
+    if (h->mpk_fused) {  // wavefront order: one launch per pass of mw_levels levels (mpk_wave.cuh)
+        cudaError_t e = cudaMemsetAsync(h->mw_sync, 0, sizeof(int) * ((size_t)h->s * h->mw_nb + 32 * (size_t)h->s + 32), sm);
+        if (e != cudaSuccess) return e;
+        for (int j0 = 0; j0 < h->s; j0 += h->mw_levels) {
+            MpkWaveParams p;
+            p.n = (int)n; p.nnz = (int)h->nnz; p.s = h->s;
+            p.j0 = j0; p.nlev = (h->s - j0 < h->mw_levels) ? h->s - j0 : h->mw_levels;
+            p.tpb = h->mw_tpb; p.nb = h->mw_nb; p.lag = h->mw_lag; p.lag_dep = h->mw_lag_dep; p.basis = h->basis;
+            p.rp = h->rp; p.ci = h->ci; p.va = h->va; p.R = R; p.AR = AR; p.st = st;
+            p.done = h->mw_sync; p.watermark = h->mw_sync + ((size_t)h->s * h->mw_nb + 31) / 32 * 32;
+            void* args[] = {&p};
+            e = cudaLaunchCooperativeKernel((const void*)mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, dim3(h->spmv_grid), dim3(BULK_WPC * 32), args,
+                                            bulk_smem_for(2, BULK_CAP, BULK_WPC), sm);
+            if (e != cudaSuccess) return e;
+            h->launches++;
+        }
+        return cudaSuccess;
+    }
     for (int j = 0; j < h->s; j++) {
         double* yjac = (j + 1 < h->s) ? R + (int64_t)(j + 1) * n : nullptr;
         int mode = 0;
@@ -392,7 +415,7 @@ void free_problem(sstep_cg* h) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
-    int** ibufs[] = {&h->perm, &h->rank, &h->own_prp, &h->own_pci};
+    int** ibufs[] = {&h->perm, &h->rank, &h->own_prp, &h->own_pci, &h->mw_sync};
     for (int** b : ibufs) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -417,7 +440,25 @@ void free_owned(sstep_cg* h) {
     h->own_va = h->own_b = h->own_x = nullptr;
 }
 
-int kernels_per_outer(const sstep_cg* h) { return h->method == 1 ? 3 : h->s + 2; }
+int kernels_per_outer(const sstep_cg* h) {
+    if (h->method == 1) return 3;
+    if (h->mpk_fused) return (h->s + h->mw_levels - 1) / h->mw_levels + 2;
+    return h->s + 2;
+}
+
+// half bandwidth in rows: max |col - row|
+__global__ void bandwidth_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci, int* __restrict__ out) {
+    const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int m = 0;
+    if (row < n)
+        for (int k = rp[row]; k < rp[row + 1]; k++) {
+            const int64_t d = (int64_t)ci[k] - row;
+            m = max(m, (int)(d < 0 ? -d : d));
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
 
 __global__ void iota_kernel(int64_t n, int* __restrict__ p) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -493,6 +534,11 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
     else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
     else if (k == "method" && (value == 0 || value == 1)) h->method = (int)value;
+    else if (k == "mpk_fused" && value >= 0 && value <= 2) h->mpk_fused_opt = (int)value;
+    else if (k == "mpk_block_rows" && value >= 0 && value % 32 == 0 && value <= (1 << 30) && ((value / 32) & (value / 32 - 1)) == 0)
+        h->mpk_block_opt = (int)value;  // 32 * 2^k rows
+    else if (k == "mpk_levels" && value >= 0 && value <= SSTEP_CG_SMAX) h->mpk_levels_opt = (int)value;
+    else if (k == "mpk_slack" && value >= -1 && value <= (1 << 20)) h->mpk_slack_opt = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -515,6 +561,12 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "launches") *value = h->launches;
     else if (k == "replace_every") *value = h->replace_every;
     else if (k == "method") *value = h->method;
+    else if (k == "mpk_fused") *value = h->mpk_fused ? 1 : 0;
+    else if (k == "bandwidth") *value = h->bandwidth;
+    else if (k == "mpk_levels_per_pass") *value = h->mw_levels;
+    else if (k == "mpk_block_rows") *value = (int64_t)h->mw_tpb * 32;
+    else if (k == "mpk_lag") *value = h->mw_lag;
+    else if (k == "mpk_lag_dep") *value = h->mw_lag_dep;
     else if (k == "reordered") *value = h->reordered ? 1 : 0;
     else if (k == "cm_levels") *value = h->cm_levels;
     else if (k == "cm_components") *value = h->cm_comps;
@@ -663,6 +715,73 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         if (want < 1) want = 1;
         cap = (int64_t)h->num_sms * 4;  // Alg. 1 kernels: two rows per thread, 4 CTAs per SM
         h->pcg_grid = (int)(want < cap ? want : cap);
+    }
+
+    // wavefront-fused MPK (mpk_wave.cuh): banded matrices on the thread-per-row bulk SpMV shape, s >= 2.  Block size B of
+    // about a quarter of the half bandwidth (at least enough tiles per step to occupy half the grid), lag = ceil(bw/B)+1,
+    // as many levels per pass as keep the re-read window (levels - 1)(bw + B) rows of CSR + vectors under 48 MB of L2.
+    h->mpk_fused = false;
+    h->mw_levels = 0;
+    // (not chosen automatically: see the measurements in mpk_wave.cuh -- it halves the DRAM traffic of the MPK but is
+    // still slower than the separate SpMVs)
+    if (h->mpk_fused_opt == 2 && h->bulk && h->lanes == 1 && h->bulk_cap == BULK_CAP && h->spmv_depth == 2 && h->form == 0 &&
+        h->method == 0 && s >= 2 && n % 4 == 0) {
+        int coop = 0;
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
+        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
+        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, h->iscratch + 3);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        h->bandwidth = hs[3];
+        // shape: small blocks (fine-grained signalling), g levels per pass, slack = 4 x the tiles the grid holds in flight
+        const int64_t gwarps = (int64_t)h->spmv_grid * BULK_WPC;
+        int64_t B = 8192;  // 256 tiles: a power of two (cheap tile decoding in the kernel)
+        if (h->mpk_block_opt) B = h->mpk_block_opt;
+        if ((B / 32) & (B / 32 - 1)) B = 0;  // not 32 * 2^k: not applicable
+        const int64_t nb = B ? (n + B - 1) / B : 0;
+        const int64_t lag_dep = B ? (h->bandwidth + B - 1) / B + 1 : 0;
+        if (!B) { coop = 0; B = 32; }
+        const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 16.0;
+        int g = s < 5 ? s : 5;  // (the kernel keeps the watermarks of up to 4 predecessor levels in registers)
+        int64_t slack = 0, lag = 0;
+        for (;; g--) {  // largest g whose re-read window (g - 1)(bw + B + slack rows) fits 48 MB of L2
+            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
+            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
+            lag = lag_dep + slack;
+            if (g <= 1 || (double)(g - 1) * (double)(lag * B) * row_bytes <= 48.0e6) break;
+        }
+        if (h->mpk_levels_opt) {
+            g = h->mpk_levels_opt < s ? h->mpk_levels_opt : s;
+            if (g > 5) g = 5;
+            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
+            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
+            lag = lag_dep + slack;
+        }
+        if (coop && g >= 2 && (nb >= 4 * lag || h->mpk_fused_opt == 2)) {
+            const int passes = (s + g - 1) / g;
+            h->mw_levels = (s + passes - 1) / passes;
+            h->mw_tpb = (int)(B / 32);
+            h->mw_nb = (int)nb;
+            h->mw_lag = (int)lag;
+            h->mw_lag_dep = (int)lag_dep;
+            cudaError_t e = cudaFuncSetAttribute(mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)bulk_smem_for(2, BULK_CAP, BULK_WPC));
+            int occ = 0;
+            if (e == cudaSuccess)
+                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, BULK_WPC * 32,
+                                                                  bulk_smem_for(2, BULK_CAP, BULK_WPC));
+            CK(e);
+            if ((int64_t)occ * h->num_sms >= h->spmv_grid) {
+                CK(cudaMalloc(&h->mw_sync, sizeof(int) * ((size_t)s * nb + 32 * (size_t)s + 32)));
+                h->mpk_fused = true;
+            }
+        }
+    }
+    if (h->mpk_fused_opt == 2 && !h->mpk_fused) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: fused matrix-powers kernel forced but not applicable (needs the thread-per-row bulk SpMV, "
+                                         "s >= 2, form = 0, n % 4 == 0 and a bandwidth whose re-read window fits L2)");
     }
 
     // resident path: whole loop in one cooperative launch when every CTA's rows fit shared memory
@@ -838,7 +957,13 @@ int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
         int e = 0;
         const int64_t n = h->n;
         for (int rep = 0; rep < reps; rep++) {
-            for (int j = 0; j < h->s; j++) {
+            if (h->mpk_fused) {  // the whole MPK is one event pair; the other s - 1 pairs stay empty
+                CK(cudaEventRecord(evs[e++], sm));
+                CK(launch_mpk(h, sm, h->R, h->AR, h->st));
+                CK(cudaEventRecord(evs[e++], sm));
+                for (int j = 1; j < h->s; j++) { CK(cudaEventRecord(evs[e++], sm)); CK(cudaEventRecord(evs[e++], sm)); }
+            }
+            for (int j = 0; j < h->s && !h->mpk_fused; j++) {
                 double* yjac = (j + 1 < h->s) ? h->R + (int64_t)(j + 1) * n : nullptr;
                 int mode = 0;
                 const double* xprev = nullptr;
