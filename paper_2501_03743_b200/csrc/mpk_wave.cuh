@@ -8,8 +8,11 @@
 // to CCTL.IVALL (L1 dropped per poll / per tile); a worker that advanced the watermark when it completed a block became
 // the straggler of the whole grid (5200 us per two levels); thousands of pollers on one address saturate its L2 slice.
 // What is left: tiles are assigned to warps statically and walked in order, so every warp is tied (within the slack) to
-// the slowest warp of the grid; ~25 % of the issued instructions are polls.  Next step: dynamic (chunked, atomically
-// claimed) tile assignment, so that slow warps simply take fewer tiles.
+// the slowest warp of the grid; ~25 % of the issued instructions are polls.  Also tried: one warp group per level (level 0
+// then never waits for anybody) -- 1360 us per level: with the warps split between the levels each level is bound by
+// the per-tile latency of its half of the warps (24 warps per SM is what 80 registers and the staging ring allow).
+// Next step: dynamic (chunked, atomically claimed) tile assignment, so that slow warps simply take fewer tiles, and a
+// leaner tile (fewer registers, more resident warps).
 //
 // The s SpMVs of the MPK sweep the same matrix s times: s (12 nnz + 4n) of the (184 s + 40) n bytes of an outer
 // iteration.  For a banded matrix (half bandwidth bw rows) level j+1 of the MPK only needs level j on the rows within
