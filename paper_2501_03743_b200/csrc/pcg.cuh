@@ -15,7 +15,8 @@
 __global__ void __launch_bounds__(256, 4)
 pcg_update_kernel(int64_t n, const double* __restrict__ p, const double* __restrict__ sk, double* __restrict__ x,
                   double* __restrict__ r, double* __restrict__ u, const double* __restrict__ dinv,
-                  const double* __restrict__ ps_partials, int nps, double* __restrict__ partials, ScgState* __restrict__ st) {
+                  const double* __restrict__ ps_partials, int nps, double* __restrict__ partials, ScgState* __restrict__ st,
+                  double dinv_uniform) {
     if (st->status != SCG_RUNNING) return;
     __shared__ double s_alpha;
     __shared__ double red[2][8];
@@ -54,14 +55,16 @@ pcg_update_kernel(int64_t n, const double* __restrict__ p, const double* __restr
         const int64_t j = i + stride;
         const double2 pa = ldg_stream2(reinterpret_cast<const double*>(p2 + i)), pb = ldg_stream2(reinterpret_cast<const double*>(p2 + j));
         const double2 sa = ldg_stream2(reinterpret_cast<const double*>(s2 + i)), sb = ldg_stream2(reinterpret_cast<const double*>(s2 + j));
-        const double2 da = d2[i], db = d2[j];
+        const double2 da = (dinv_uniform > 0.0) ? make_double2(dinv_uniform, dinv_uniform) : d2[i];
+        const double2 db = (dinv_uniform > 0.0) ? da : d2[j];
         const double2 xa = x2[i], xb = x2[j];
         const double2 ra = r2[i], rb = r2[j];
         one(pa, sa, da, xa, ra, i);
         one(pb, sb, db, xb, rb, j);
     }
     if (i < n2)
-        one(ldg_stream2(reinterpret_cast<const double*>(p2 + i)), ldg_stream2(reinterpret_cast<const double*>(s2 + i)), d2[i], x2[i], r2[i], i);
+        one(ldg_stream2(reinterpret_cast<const double*>(p2 + i)), ldg_stream2(reinterpret_cast<const double*>(s2 + i)),
+            (dinv_uniform > 0.0) ? make_double2(dinv_uniform, dinv_uniform) : d2[i], x2[i], r2[i], i);
     if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
         const int64_t row = n - 1;
         const double xi = fma(alpha, p[row], x[row]);

@@ -70,6 +70,7 @@ struct sstep_cg {
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int64_t num_tiles = 0;
     int max_row_len = 0;
+    double dinv_uniform = 0.0;  // 1 / a_ii if the diagonal is constant (then the update kernels skip the dinv stream), else 0
     // locality reordering (reorder.cuh): A' = Pi A Pi^T in owned arrays; rp/ci/va above then point at them
     bool reordered = false;
     int *perm = nullptr, *rank = nullptr;        // perm[new] = old, rank[old] = new
@@ -269,7 +270,7 @@ cudaError_t update_SM(sstep_cg* h, cudaStream_t sm, bool configure, double* R, c
         update_tma_kernel<S, MOM><<<h->update_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
                                                                                  h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
     } else {
-        update_kernel<S, MOM><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out);
+        update_kernel<S, MOM><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out, h->dinv_uniform);
     }
     return cudaGetLastError();
 }
@@ -387,7 +388,7 @@ cudaError_t launch_pcg_iteration(sstep_cg* h, cudaStream_t sm, cudaEvent_t* evs 
     if (e != cudaSuccess) return e;
     if (evs) { cudaEventRecord(evs[1], sm); cudaEventRecord(evs[2], sm); }
     pcg_update_kernel<<<h->pcg_grid, 256, 0, sm>>>(h->n, h->P, h->AP, h->x, h->r, h->R, h->dinv, h->mom, h->spmv_grid,
-                                                         h->partials, h->st);
+                                                         h->partials, h->st, h->dinv_uniform);
     if (evs) { cudaEventRecord(evs[3], sm); cudaEventRecord(evs[4], sm); }
     pcg_direction_kernel<<<h->pcg_grid, 256, 0, sm>>>(h->n, h->R, h->P, h->st);
     if (evs) cudaEventRecord(evs[5], sm);
@@ -563,6 +564,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "method") *value = h->method;
     else if (k == "mpk_fused") *value = h->mpk_fused ? 1 : 0;
     else if (k == "bandwidth") *value = h->bandwidth;
+    else if (k == "uniform_diagonal") *value = h->dinv_uniform > 0.0 ? 1 : 0;
     else if (k == "mpk_levels_per_pass") *value = h->mw_levels;
     else if (k == "mpk_block_rows") *value = (int64_t)h->mw_tpb * 32;
     else if (k == "mpk_lag") *value = h->mw_lag;
@@ -660,6 +662,18 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
         }
     }
 
+    // constant diagonal?  (all Poisson configs: the update kernels then take 1 / a_ii as a scalar)
+    {
+        int one = 1, flag = 0;
+        double d0 = 0.0;
+        CK(cudaMemcpyAsync(h->iscratch + 3, &one, sizeof(int), cudaMemcpyHostToDevice, sm));
+        uniform_diag_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, h->dinv, h->iscratch + 3);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(&flag, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaMemcpyAsync(&d0, h->dinv, sizeof(double), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        h->dinv_uniform = (flag == 1 && d0 > 0.0) ? d0 : 0.0;
+    }
     // SpMV variant: lanes per row from the mean row length (vector-per-row ... warp-per-row), bulk staging if every tile fits
     const double mean = (double)nnz / (double)n;
     int L = 1;

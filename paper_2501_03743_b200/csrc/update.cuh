@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(256, (S <= 2) ? 4 : 2)
 update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
-              ScgState* __restrict__ st, double* __restrict__ rho_out) {
+              ScgState* __restrict__ st, double* __restrict__ rho_out, double dinv_uniform) {
     if (st->status != SCG_RUNNING) return;
     __shared__ __align__(16) double sbeta[S * S];
     __shared__ double salpha[S];
@@ -150,7 +150,8 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
     double rho = 0.0, mu0 = 0.0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; row < n; row += stride) {
-        const double x0 = x[row], r0 = r[row], di = dinv[row];
+        // (a constant diagonal -- every Poisson config -- needs no dinv stream: 8n bytes less per update)
+        const double x0 = x[row], r0 = r[row], di = (dinv_uniform > 0.0) ? dinv_uniform : dinv[row];
         const double xi = update_half<S>(n, row, R, P, sbeta, salpha, x0, 1.0);     // P <- R + P beta ; x += P alpha
         const double ri = update_half<S>(n, row, AR, AP, sbeta, salpha, r0, -1.0);  // AP <- AR + AP beta ; r -= AP alpha
         x[row] = xi;
@@ -234,6 +235,13 @@ init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ 
             st->ticket_update = 0;
         }
     }
+}
+
+// ---- setup: is the diagonal constant?  flag[0] stays 1 if every dinv[i] has the bits of dinv[0]
+__global__ void uniform_diag_kernel(int64_t n, const double* __restrict__ dinv, int* __restrict__ flag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool bad = (i < n) && (dinv[i] != dinv[0]);
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicAnd(flag, 0);
 }
 
 // ---- setup: dinv = 1/a_ii, structural validation, row-length statistics ----
