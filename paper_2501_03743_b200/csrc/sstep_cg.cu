@@ -466,6 +466,347 @@ __global__ void iota_kernel(int64_t n, int* __restrict__ p) {
     if (i < n) p[i] = (int)i;
 }
 
+// ---------------------------------------------------------------- the steps of sstep_cg_setup (each returns 0 or an error code)
+// validation of the CSR arrays, dinv = 1 / a_ii, longest row
+int setup_analyze(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int64_t nnz = h->nnz;
+    cudaStream_t sm = h->stream;
+    const int* rowptr = h->rp;
+    const int* colidx = h->ci;
+    const double* vals = h->va;
+    int hs[4] = {0, 0, 0, 0};
+    CK(cudaMalloc(&h->dinv, sizeof(double) * n));
+    CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
+    analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
+    CK(cudaStreamSynchronize(sm));
+    if (hs[0]) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "setup: invalid matrix (flags %d: 1 rowptr, 2 column index, 4 diagonal missing or <= 0)", hs[0]);
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_MATRIX, buf);
+    }
+    h->max_row_len = hs[1];
+    return 0;
+}
+
+// locality test and, if wanted, the Cuthill-McKee renumbering (h->rp / ci / va then point at the owned permuted copy)
+int setup_reorder(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int64_t nnz = h->nnz;
+    cudaStream_t sm = h->stream;
+    const int* rowptr = h->rp;
+    const int* colidx = h->ci;
+    const double* vals = h->va;
+    int hs[4] = {0, 0, 0, 0};
+    // auto: only when the gathered vector cannot live in L2 (n >= 2^23 rows = 67 MB) and more than a quarter of the
+    // entries reach further than 2^20 rows (8 MB) from the diagonal
+    {
+        unsigned long long* far = nullptr;
+        unsigned long long hfar = 0;
+        CK(cudaMalloc(&far, sizeof(unsigned long long)));
+        CK(cudaMemsetAsync(far, 0, sizeof(unsigned long long), sm));
+        scg_reorder::far_entries_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, 1 << 20, far);
+        CK(cudaMemcpyAsync(&hfar, far, sizeof(unsigned long long), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        cudaFree(far);
+        h->far_permille = (int)(1000.0 * (double)hfar / (double)nnz);
+    }
+    h->cm_levels = h->cm_comps = 0;
+    if (h->reorder_opt == 2 || (h->reorder_opt == 0 && n >= (int64_t(1) << 23) && h->far_permille > 250)) {
+        CK(cudaMalloc(&h->perm, sizeof(int) * (size_t)n));
+        CK(cudaMalloc(&h->rank, sizeof(int) * (size_t)n));
+        bool done = false;
+        CK(scg_reorder::cuthill_mckee((int)n, rowptr, colidx, sm, h->perm, h->rank, &done, &h->cm_levels, &h->cm_comps));
+        if (done) {
+            CK(cudaMalloc(&h->own_prp, sizeof(int) * ((size_t)n + 1)));
+            CK(cudaMalloc(&h->own_pci, sizeof(int) * (size_t)nnz));
+            CK(cudaMalloc(&h->own_pva, sizeof(double) * (size_t)nnz));
+            CK(cudaMalloc(&h->bperm, sizeof(double) * (size_t)n));
+            CK(cudaMalloc(&h->x0perm, sizeof(double) * (size_t)n));
+            CK(scg_reorder::permute_csr((int)n, (int)nnz, h->perm, h->rank, rowptr, colidx, vals, h->own_prp, h->own_pci, h->own_pva, sm));
+            h->rp = rowptr = h->own_prp;
+            h->ci = colidx = h->own_pci;
+            h->va = vals = h->own_pva;
+            h->reordered = true;
+            // dinv and the row statistics of the permuted matrix (same validation, now of our own copy)
+            CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
+            analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+            if (hs[0]) {
+                free_problem(h);
+                return fail(h, SSTEP_CG_ERR_CUDA, "setup: internal error, the permuted matrix failed validation");
+            }
+        } else {
+            cudaFree(h->perm); cudaFree(h->rank);
+            h->perm = h->rank = nullptr;
+        }
+    }
+    return 0;
+}
+
+// is the diagonal constant?
+int setup_uniform_diagonal(sstep_cg* h) {
+    const int64_t n = h->n;
+    cudaStream_t sm = h->stream;
+    {
+        int one = 1, flag = 0;
+        double d0 = 0.0;
+        CK(cudaMemcpyAsync(h->iscratch + 3, &one, sizeof(int), cudaMemcpyHostToDevice, sm));
+        uniform_diag_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, h->dinv, h->iscratch + 3);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(&flag, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaMemcpyAsync(&d0, h->dinv, sizeof(double), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        h->dinv_uniform = (flag == 1 && d0 > 0.0) ? d0 : 0.0;
+    }
+    return 0;
+}
+
+// lanes per row and generic / bulk-staged SpMV (tile shape) from the row statistics
+int setup_spmv_variant(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int64_t nnz = h->nnz;
+    cudaStream_t sm = h->stream;
+    const int* rowptr = h->rp;
+    const int* colidx = h->ci;
+    const double* vals = h->va;
+    int hs[4] = {0, 0, 0, 0};
+    const double mean = (double)nnz / (double)n;
+    int L = 1;
+    while (L < 32 && mean / L > 8.0) L *= 2;
+    if (h->lanes_opt) L = h->lanes_opt;
+    h->bulk = false;
+    const bool aligned = (((uintptr_t)colidx | (uintptr_t)vals) & 15) == 0;
+    // auto: the bulk-staged kernel for thread-per-row matrices (mean row <= 8 entries, e.g. 7-point stencils), where it
+    // reaches the copy peak, and -- with TWO lanes per row and 512-entry tiles -- for mean rows of 16..32 entries
+    // (27-point 160^3: 257 us against 272 us for the generic kernel at L = 4 and 285 us for bulk tiles at L = 4: few lanes
+    // per row keep the x gathers of a warp on consecutive addresses).  Forced (spmv_variant = 2): any L whose tiles fit.
+    const bool auto_bulk = h->spmv_variant == 0 && (L == 1 || (L == 4 && !h->lanes_opt && h->spmv_depth == 2));
+    if ((h->spmv_variant == 2 || auto_bulk) && aligned && n + 64 < (int64_t(1) << 31)) {
+        if (auto_bulk && L == 4) L = 2;
+        for (int Lb = L; Lb <= 32; Lb *= 2) {
+            const int rpt = 32 / Lb;
+            const int64_t tiles = (n + rpt - 1) / rpt;
+            CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
+            tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, rpt, tiles, h->iscratch + 2);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+            int cap = 0, wpc = BULK_WPC;
+            if (hs[2] + 3 <= BULK_CAP) cap = BULK_CAP;
+            else if (Lb == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP2) { cap = BULK_CAP2; wpc = BULK_WPC2; }
+            else if (Lb == 1 && h->spmv_variant == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP1) { cap = BULK_CAP1; wpc = BULK_WPC1; }
+            if (cap) {
+                h->bulk = true;
+                h->bulk_cap = cap;
+                h->bulk_wpc = wpc;
+                L = Lb;
+                h->num_tiles = tiles;
+                break;
+            }
+            if (h->lanes_opt || h->spmv_variant == 0) break;
+        }
+        if (auto_bulk && !h->bulk && L == 2) L = 4;  // tiles too large: back to the generic kernel at its own L
+    }
+    if (h->spmv_variant == 2 && !h->bulk) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: bulk SpMV forced but a tile exceeds the staging capacity or arrays are not 16 B aligned");
+    }
+    h->lanes = L;
+    return 0;
+}
+
+// grids of the Gram / update / init / Alg. 1 kernels
+int setup_block_kernels(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int s = h->s;
+    cudaStream_t sm = h->stream;
+    h->staged = (h->block_variant == 2) || (h->block_variant == 0 && s >= 5);
+    CK(config_spmv(h));
+    CK(launch_gram(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, 0));
+    CK(launch_update(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr));
+    {
+        int64_t want = (n + 255) / 256, cap = (int64_t)h->num_sms * 8;
+        h->init_grid = (int)(want < cap ? want : cap);
+        want = (n / 2 + 255) / 256;
+        if (want < 1) want = 1;
+        cap = (int64_t)h->num_sms * 4;  // Alg. 1 kernels: two rows per thread, 4 CTAs per SM
+        h->pcg_grid = (int)(want < cap ? want : cap);
+    }
+    return 0;
+}
+
+// shape of the experimental wavefront-fused matrix-powers kernel
+int setup_mpk_wave(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int64_t nnz = h->nnz;
+    const int s = h->s;
+    cudaStream_t sm = h->stream;
+    const int* rowptr = h->rp;
+    const int* colidx = h->ci;
+    int hs[4] = {0, 0, 0, 0};
+    // banded matrices on the thread-per-row bulk SpMV shape, s >= 2: blocks of 8192 rows, dependency distance
+    // ceil(bw / B) + 1 blocks plus a slack, as many levels per pass as keep the re-read window under 48 MB of L2
+    h->mpk_fused = false;
+    h->mw_levels = 0;
+    // (not chosen automatically: see the measurements in mpk_wave.cuh -- it halves the DRAM traffic of the MPK but is
+    // still slower than the separate SpMVs)
+    if (h->mpk_fused_opt == 2 && h->bulk && h->lanes == 1 && h->bulk_cap == BULK_CAP && h->spmv_depth == 2 && h->form == 0 &&
+        h->method == 0 && s >= 2 && n % 4 == 0) {
+        int coop = 0;
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
+        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
+        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, h->iscratch + 3);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        h->bandwidth = hs[3];
+        // shape: small blocks (fine-grained signalling), g levels per pass, slack = 4 x the tiles the grid holds in flight
+        const int64_t gwarps = (int64_t)h->spmv_grid * BULK_WPC;
+        int64_t B = 8192;  // 256 tiles: a power of two (cheap tile decoding in the kernel)
+        if (h->mpk_block_opt) B = h->mpk_block_opt;
+        if ((B / 32) & (B / 32 - 1)) B = 0;  // not 32 * 2^k: not applicable
+        const int64_t nb = B ? (n + B - 1) / B : 0;
+        const int64_t lag_dep = B ? (h->bandwidth + B - 1) / B + 1 : 0;
+        if (!B) { coop = 0; B = 32; }
+        const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 16.0;
+        int g = s < 5 ? s : 5;  // (the kernel keeps the watermarks of up to 4 predecessor levels in registers)
+        int64_t slack = 0, lag = 0;
+        for (;; g--) {  // largest g whose re-read window (g - 1)(bw + B + slack rows) fits 48 MB of L2
+            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
+            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
+            lag = lag_dep + slack;
+            if (g <= 1 || (double)(g - 1) * (double)(lag * B) * row_bytes <= 48.0e6) break;
+        }
+        if (h->mpk_levels_opt) {
+            g = h->mpk_levels_opt < s ? h->mpk_levels_opt : s;
+            if (g > 5) g = 5;
+            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
+            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
+            lag = lag_dep + slack;
+        }
+        if (coop && g >= 2 && (nb >= 4 * lag || h->mpk_fused_opt == 2)) {
+            const int passes = (s + g - 1) / g;
+            h->mw_levels = (s + passes - 1) / passes;
+            h->mw_tpb = (int)(B / 32);
+            h->mw_nb = (int)nb;
+            h->mw_lag = (int)lag;
+            h->mw_lag_dep = (int)lag_dep;
+            cudaError_t e = cudaFuncSetAttribute(mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)bulk_smem_for(2, BULK_CAP, BULK_WPC));
+            int occ = 0;
+            if (e == cudaSuccess)
+                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, BULK_WPC * 32,
+                                                                  bulk_smem_for(2, BULK_CAP, BULK_WPC));
+            CK(e);
+            if ((int64_t)occ * h->num_sms >= h->spmv_grid) {
+                CK(cudaMalloc(&h->mw_sync, sizeof(int) * ((size_t)s * nb + 32 * (size_t)s + 32)));
+                h->mpk_fused = true;
+            }
+        }
+    }
+    if (h->mpk_fused_opt == 2 && !h->mpk_fused) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: fused matrix-powers kernel forced but not applicable (needs the thread-per-row bulk SpMV, "
+                                         "s >= 2, form = 0, n % 4 == 0 and a bandwidth whose re-read window fits L2)");
+    }
+    return 0;
+}
+
+// eligibility and shape of the resident (whole loop in one cooperative launch) path
+int setup_resident(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int s = h->s;
+    cudaStream_t sm = h->stream;
+    const int* rowptr = h->rp;
+    int hs[4] = {0, 0, 0, 0};
+    h->resident = false;
+    h->res_grid = 0;
+    // (auto: s <= 4 only -- above, the redundant per-CTA reduction of the 2s^2+s partials outweighs the saved launches)
+    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && h->replace_every == 0 && h->method == 0 && n + 4096 < (int64_t(1) << 31)) {
+        int coop = 0;
+        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
+        int64_t g = (n + 31) / 32;
+        if (g > h->num_sms) g = h->num_sms;
+        int64_t rpb = ((n + g - 1) / g + 31) / 32 * 32;
+        g = (n + rpb - 1) / rpb;
+        // (the vectors alone must fit: skips the tile scan for every problem that is far too large)
+        if (resident_smem_bytes(s, (int)(rpb < (1 << 20) ? rpb : (1 << 20)), 0) > (size_t)200 * 1024) coop = 0;
+        if (coop) {
+            CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
+            tile_nnz_max_kernel<<<(unsigned)((g + 255) / 256), 256, 0, sm>>>(n, rowptr, (int)rpb, g, h->iscratch + 3);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
+            CK(cudaStreamSynchronize(sm));
+        }
+        const int nzcap = (hs[3] + 3) & ~3;
+        const size_t bytes = coop ? resident_smem_bytes(s, (int)rpb, nzcap) : 0;
+        if (coop && bytes <= (size_t)200 * 1024) {
+            h->res_grid = (int)g; h->res_rpb = (int)rpb; h->res_nzcap = nzcap; h->res_smem = bytes;
+            h->res_threads = (int)(rpb < 512 ? rpb : 512);
+            int occ = 0;
+            CK(resident_op(h, sm, 0, 0, &occ));
+            h->resident = occ >= 1 && (int64_t)occ * h->num_sms >= g;
+        }
+        if (!h->resident) h->res_grid = 0;
+    }
+    if (h->resident_opt == 2 && !h->resident) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: resident path forced but the problem does not fit shared memory (or form = 1 / replace_every > 0)");
+    }
+    return 0;
+}
+
+// workspaces: R, AR, P, AP, x, r, partial-sum scratch
+int setup_workspaces(sstep_cg* h) {
+    const int64_t n = h->n;
+    const int s = h->s;
+    cudaStream_t sm = h->stream;
+    const size_t blk = sizeof(double) * (size_t)n * s;
+    CK(cudaMalloc(&h->R, blk));
+    CK(cudaMalloc(&h->AR, blk));
+    CK(cudaMalloc(&h->P, blk));
+    CK(cudaMalloc(&h->AP, blk));
+    CK(cudaMalloc(&h->x, sizeof(double) * n));
+    CK(cudaMalloc(&h->r, sizeof(double) * n));
+    size_t np = (size_t)h->gram_grid * (2 * s * s + s);
+    if (np < 2 * (size_t)h->update_grid) np = 2 * (size_t)h->update_grid;
+    if (np < 2 * (size_t)h->init_grid) np = 2 * (size_t)h->init_grid;
+    if (np < 2 * (size_t)h->pcg_grid) np = 2 * (size_t)h->pcg_grid;
+    if (np < (size_t)h->res_grid * (2 * s * s + s + 1)) np = (size_t)h->res_grid * (2 * s * s + s + 1);
+    CK(cudaMalloc(&h->partials, sizeof(double) * np));
+    CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
+    CK(cudaMemsetAsync(h->mom, 0, sizeof(double) * 2 * s * (size_t)h->spmv_grid, sm));
+    CK(cudaMemsetAsync(h->R, 0, blk, sm));
+    CK(cudaMemsetAsync(h->AR, 0, blk, sm));
+    CK(cudaMemsetAsync(h->P, 0, blk, sm));
+    CK(cudaMemsetAsync(h->AP, 0, blk, sm));
+    CK(cudaMemsetAsync(h->st, 0, sizeof(ScgState), sm));
+    CK(cudaMemsetAsync(h->st_test, 0, sizeof(ScgState), sm));
+    CK(cudaStreamSynchronize(sm));
+    return 0;
+}
+
+// capture of one outer iteration into a CUDA graph
+int setup_graph(sstep_cg* h) {
+    if (h->use_graph) {
+        const int64_t saved = h->launches;
+        CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+        cudaError_t e = launch_outer(h, h->cap_stream);
+        cudaError_t e2 = cudaStreamEndCapture(h->cap_stream, &h->graph);
+        h->launches = saved;
+        if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        CK(e2);
+        CK(cudaGraphInstantiate(&h->gexec, h->graph, 0));
+    }
+    return 0;
+}
+
 }  // namespace
 
 // =============================================================================================== C ABI
@@ -598,277 +939,16 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     free_problem(h);
     h->n = n; h->nnz = nnz; h->s = s;
     h->rp = rowptr; h->ci = colidx; h->va = vals;
-    cudaStream_t sm = h->stream;
 
-    // dinv, validation, row statistics
-    CK(cudaMalloc(&h->dinv, sizeof(double) * n));
-    CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
-    analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
-    CK(cudaGetLastError());
-    int hs[4] = {0, 0, 0, 0};
-    CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
-    CK(cudaStreamSynchronize(sm));
-    if (hs[0]) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "setup: invalid matrix (flags %d: 1 rowptr, 2 column index, 4 diagonal missing or <= 0)", hs[0]);
-        free_problem(h);
-        return fail(h, SSTEP_CG_ERR_MATRIX, buf);
-    }
-    h->max_row_len = hs[1];
-
-    // locality reordering (reorder.cuh).  auto: only when the gathered vector cannot live in L2 (n >= 2^23 rows = 67 MB)
-    // and more than a quarter of the entries reach further than 2^20 rows (8 MB) from the diagonal.
-    {
-        unsigned long long* far = nullptr;
-        unsigned long long hfar = 0;
-        CK(cudaMalloc(&far, sizeof(unsigned long long)));
-        CK(cudaMemsetAsync(far, 0, sizeof(unsigned long long), sm));
-        scg_reorder::far_entries_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, 1 << 20, far);
-        CK(cudaMemcpyAsync(&hfar, far, sizeof(unsigned long long), cudaMemcpyDeviceToHost, sm));
-        CK(cudaStreamSynchronize(sm));
-        cudaFree(far);
-        h->far_permille = (int)(1000.0 * (double)hfar / (double)nnz);
-    }
-    h->cm_levels = h->cm_comps = 0;
-    if (h->reorder_opt == 2 || (h->reorder_opt == 0 && n >= (int64_t(1) << 23) && h->far_permille > 250)) {
-        CK(cudaMalloc(&h->perm, sizeof(int) * (size_t)n));
-        CK(cudaMalloc(&h->rank, sizeof(int) * (size_t)n));
-        bool done = false;
-        CK(scg_reorder::cuthill_mckee((int)n, rowptr, colidx, sm, h->perm, h->rank, &done, &h->cm_levels, &h->cm_comps));
-        if (done) {
-            CK(cudaMalloc(&h->own_prp, sizeof(int) * ((size_t)n + 1)));
-            CK(cudaMalloc(&h->own_pci, sizeof(int) * (size_t)nnz));
-            CK(cudaMalloc(&h->own_pva, sizeof(double) * (size_t)nnz));
-            CK(cudaMalloc(&h->bperm, sizeof(double) * (size_t)n));
-            CK(cudaMalloc(&h->x0perm, sizeof(double) * (size_t)n));
-            CK(scg_reorder::permute_csr((int)n, (int)nnz, h->perm, h->rank, rowptr, colidx, vals, h->own_prp, h->own_pci, h->own_pva, sm));
-            h->rp = rowptr = h->own_prp;
-            h->ci = colidx = h->own_pci;
-            h->va = vals = h->own_pva;
-            h->reordered = true;
-            // dinv and the row statistics of the permuted matrix (same validation, now of our own copy)
-            CK(cudaMemsetAsync(h->iscratch, 0, 4 * sizeof(int), sm));
-            analyze_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, nnz, rowptr, colidx, vals, h->dinv, h->iscratch, h->iscratch + 1);
-            CK(cudaGetLastError());
-            CK(cudaMemcpyAsync(hs, h->iscratch, 2 * sizeof(int), cudaMemcpyDeviceToHost, sm));
-            CK(cudaStreamSynchronize(sm));
-            if (hs[0]) {
-                free_problem(h);
-                return fail(h, SSTEP_CG_ERR_CUDA, "setup: internal error, the permuted matrix failed validation");
-            }
-        } else {
-            cudaFree(h->perm); cudaFree(h->rank);
-            h->perm = h->rank = nullptr;
-        }
-    }
-
-    // constant diagonal?  (all Poisson configs: the update kernels then take 1 / a_ii as a scalar)
-    {
-        int one = 1, flag = 0;
-        double d0 = 0.0;
-        CK(cudaMemcpyAsync(h->iscratch + 3, &one, sizeof(int), cudaMemcpyHostToDevice, sm));
-        uniform_diag_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, h->dinv, h->iscratch + 3);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(&flag, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
-        CK(cudaMemcpyAsync(&d0, h->dinv, sizeof(double), cudaMemcpyDeviceToHost, sm));
-        CK(cudaStreamSynchronize(sm));
-        h->dinv_uniform = (flag == 1 && d0 > 0.0) ? d0 : 0.0;
-    }
-    // SpMV variant: lanes per row from the mean row length (vector-per-row ... warp-per-row), bulk staging if every tile fits
-    const double mean = (double)nnz / (double)n;
-    int L = 1;
-    while (L < 32 && mean / L > 8.0) L *= 2;
-    if (h->lanes_opt) L = h->lanes_opt;
-    h->bulk = false;
-    const bool aligned = (((uintptr_t)colidx | (uintptr_t)vals) & 15) == 0;
-    // auto: the bulk-staged kernel for thread-per-row matrices (mean row <= 8 entries, e.g. 7-point stencils), where it
-    // reaches the copy peak, and -- with TWO lanes per row and 512-entry tiles -- for mean rows of 16..32 entries
-    // (27-point 160^3: 257 us against 272 us for the generic kernel at L = 4 and 285 us for bulk tiles at L = 4: few lanes
-    // per row keep the x gathers of a warp on consecutive addresses).  Forced (spmv_variant = 2): any L whose tiles fit.
-    const bool auto_bulk = h->spmv_variant == 0 && (L == 1 || (L == 4 && !h->lanes_opt && h->spmv_depth == 2));
-    if ((h->spmv_variant == 2 || auto_bulk) && aligned && n + 64 < (int64_t(1) << 31)) {
-        if (auto_bulk && L == 4) L = 2;
-        for (int Lb = L; Lb <= 32; Lb *= 2) {
-            const int rpt = 32 / Lb;
-            const int64_t tiles = (n + rpt - 1) / rpt;
-            CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
-            tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, rpt, tiles, h->iscratch + 2);
-            CK(cudaGetLastError());
-            CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
-            CK(cudaStreamSynchronize(sm));
-            int cap = 0, wpc = BULK_WPC;
-            if (hs[2] + 3 <= BULK_CAP) cap = BULK_CAP;
-            else if (Lb == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP2) { cap = BULK_CAP2; wpc = BULK_WPC2; }
-            else if (Lb == 1 && h->spmv_variant == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP1) { cap = BULK_CAP1; wpc = BULK_WPC1; }
-            if (cap) {
-                h->bulk = true;
-                h->bulk_cap = cap;
-                h->bulk_wpc = wpc;
-                L = Lb;
-                h->num_tiles = tiles;
-                break;
-            }
-            if (h->lanes_opt || h->spmv_variant == 0) break;
-        }
-        if (auto_bulk && !h->bulk && L == 2) L = 4;  // tiles too large: back to the generic kernel at its own L
-    }
-    if (h->spmv_variant == 2 && !h->bulk) {
-        free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: bulk SpMV forced but a tile exceeds the staging capacity or arrays are not 16 B aligned");
-    }
-    h->lanes = L;
-    // Gram / update: register kernels for s <= 4 (they reach the copy peak), TMA tile pipeline above
-    h->staged = (h->block_variant == 2) || (h->block_variant == 0 && s >= 5);
-    CK(config_spmv(h));
-    CK(launch_gram(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, 0));
-    CK(launch_update(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr));
-    {
-        int64_t want = (n + 255) / 256, cap = (int64_t)h->num_sms * 8;
-        h->init_grid = (int)(want < cap ? want : cap);
-        want = (n / 2 + 255) / 256;
-        if (want < 1) want = 1;
-        cap = (int64_t)h->num_sms * 4;  // Alg. 1 kernels: two rows per thread, 4 CTAs per SM
-        h->pcg_grid = (int)(want < cap ? want : cap);
-    }
-
-    // wavefront-fused MPK (mpk_wave.cuh): banded matrices on the thread-per-row bulk SpMV shape, s >= 2.  Block size B of
-    // about a quarter of the half bandwidth (at least enough tiles per step to occupy half the grid), lag = ceil(bw/B)+1,
-    // as many levels per pass as keep the re-read window (levels - 1)(bw + B) rows of CSR + vectors under 48 MB of L2.
-    h->mpk_fused = false;
-    h->mw_levels = 0;
-    // (not chosen automatically: see the measurements in mpk_wave.cuh -- it halves the DRAM traffic of the MPK but is
-    // still slower than the separate SpMVs)
-    if (h->mpk_fused_opt == 2 && h->bulk && h->lanes == 1 && h->bulk_cap == BULK_CAP && h->spmv_depth == 2 && h->form == 0 &&
-        h->method == 0 && s >= 2 && n % 4 == 0) {
-        int coop = 0;
-        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
-        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
-        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, h->iscratch + 3);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
-        CK(cudaStreamSynchronize(sm));
-        h->bandwidth = hs[3];
-        // shape: small blocks (fine-grained signalling), g levels per pass, slack = 4 x the tiles the grid holds in flight
-        const int64_t gwarps = (int64_t)h->spmv_grid * BULK_WPC;
-        int64_t B = 8192;  // 256 tiles: a power of two (cheap tile decoding in the kernel)
-        if (h->mpk_block_opt) B = h->mpk_block_opt;
-        if ((B / 32) & (B / 32 - 1)) B = 0;  // not 32 * 2^k: not applicable
-        const int64_t nb = B ? (n + B - 1) / B : 0;
-        const int64_t lag_dep = B ? (h->bandwidth + B - 1) / B + 1 : 0;
-        if (!B) { coop = 0; B = 32; }
-        const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 16.0;
-        int g = s < 5 ? s : 5;  // (the kernel keeps the watermarks of up to 4 predecessor levels in registers)
-        int64_t slack = 0, lag = 0;
-        for (;; g--) {  // largest g whose re-read window (g - 1)(bw + B + slack rows) fits 48 MB of L2
-            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
-            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
-            lag = lag_dep + slack;
-            if (g <= 1 || (double)(g - 1) * (double)(lag * B) * row_bytes <= 48.0e6) break;
-        }
-        if (h->mpk_levels_opt) {
-            g = h->mpk_levels_opt < s ? h->mpk_levels_opt : s;
-            if (g > 5) g = 5;
-            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
-            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
-            lag = lag_dep + slack;
-        }
-        if (coop && g >= 2 && (nb >= 4 * lag || h->mpk_fused_opt == 2)) {
-            const int passes = (s + g - 1) / g;
-            h->mw_levels = (s + passes - 1) / passes;
-            h->mw_tpb = (int)(B / 32);
-            h->mw_nb = (int)nb;
-            h->mw_lag = (int)lag;
-            h->mw_lag_dep = (int)lag_dep;
-            cudaError_t e = cudaFuncSetAttribute(mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 (int)bulk_smem_for(2, BULK_CAP, BULK_WPC));
-            int occ = 0;
-            if (e == cudaSuccess)
-                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, BULK_WPC * 32,
-                                                                  bulk_smem_for(2, BULK_CAP, BULK_WPC));
-            CK(e);
-            if ((int64_t)occ * h->num_sms >= h->spmv_grid) {
-                CK(cudaMalloc(&h->mw_sync, sizeof(int) * ((size_t)s * nb + 32 * (size_t)s + 32)));
-                h->mpk_fused = true;
-            }
-        }
-    }
-    if (h->mpk_fused_opt == 2 && !h->mpk_fused) {
-        free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: fused matrix-powers kernel forced but not applicable (needs the thread-per-row bulk SpMV, "
-                                         "s >= 2, form = 0, n % 4 == 0 and a bandwidth whose re-read window fits L2)");
-    }
-
-    // resident path: whole loop in one cooperative launch when every CTA's rows fit shared memory
-    h->resident = false;
-    h->res_grid = 0;
-    // (auto: s <= 4 only -- above, the redundant per-CTA reduction of the 2s^2+s partials outweighs the saved launches)
-    if (h->resident_opt != 1 && (h->resident_opt == 2 || s <= 4) && h->form == 0 && h->replace_every == 0 && h->method == 0 && n + 4096 < (int64_t(1) << 31)) {
-        int coop = 0;
-        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
-        int64_t g = (n + 31) / 32;
-        if (g > h->num_sms) g = h->num_sms;
-        int64_t rpb = ((n + g - 1) / g + 31) / 32 * 32;
-        g = (n + rpb - 1) / rpb;
-        // (the vectors alone must fit: skips the tile scan for every problem that is far too large)
-        if (resident_smem_bytes(s, (int)(rpb < (1 << 20) ? rpb : (1 << 20)), 0) > (size_t)200 * 1024) coop = 0;
-        if (coop) {
-            CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
-            tile_nnz_max_kernel<<<(unsigned)((g + 255) / 256), 256, 0, sm>>>(n, rowptr, (int)rpb, g, h->iscratch + 3);
-            CK(cudaGetLastError());
-            CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
-            CK(cudaStreamSynchronize(sm));
-        }
-        const int nzcap = (hs[3] + 3) & ~3;
-        const size_t bytes = coop ? resident_smem_bytes(s, (int)rpb, nzcap) : 0;
-        if (coop && bytes <= (size_t)200 * 1024) {
-            h->res_grid = (int)g; h->res_rpb = (int)rpb; h->res_nzcap = nzcap; h->res_smem = bytes;
-            h->res_threads = (int)(rpb < 512 ? rpb : 512);
-            int occ = 0;
-            CK(resident_op(h, sm, 0, 0, &occ));
-            h->resident = occ >= 1 && (int64_t)occ * h->num_sms >= g;
-        }
-        if (!h->resident) h->res_grid = 0;
-    }
-    if (h->resident_opt == 2 && !h->resident) {
-        free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: resident path forced but the problem does not fit shared memory (or form = 1 / replace_every > 0)");
-    }
-
-    // workspaces
-    const size_t blk = sizeof(double) * (size_t)n * s;
-    CK(cudaMalloc(&h->R, blk));
-    CK(cudaMalloc(&h->AR, blk));
-    CK(cudaMalloc(&h->P, blk));
-    CK(cudaMalloc(&h->AP, blk));
-    CK(cudaMalloc(&h->x, sizeof(double) * n));
-    CK(cudaMalloc(&h->r, sizeof(double) * n));
-    size_t np = (size_t)h->gram_grid * (2 * s * s + s);
-    if (np < 2 * (size_t)h->update_grid) np = 2 * (size_t)h->update_grid;
-    if (np < 2 * (size_t)h->init_grid) np = 2 * (size_t)h->init_grid;
-    if (np < 2 * (size_t)h->pcg_grid) np = 2 * (size_t)h->pcg_grid;
-    if (np < (size_t)h->res_grid * (2 * s * s + s + 1)) np = (size_t)h->res_grid * (2 * s * s + s + 1);
-    CK(cudaMalloc(&h->partials, sizeof(double) * np));
-    CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
-    CK(cudaMemsetAsync(h->mom, 0, sizeof(double) * 2 * s * (size_t)h->spmv_grid, sm));
-    CK(cudaMemsetAsync(h->R, 0, blk, sm));
-    CK(cudaMemsetAsync(h->AR, 0, blk, sm));
-    CK(cudaMemsetAsync(h->P, 0, blk, sm));
-    CK(cudaMemsetAsync(h->AP, 0, blk, sm));
-    CK(cudaMemsetAsync(h->st, 0, sizeof(ScgState), sm));
-    CK(cudaMemsetAsync(h->st_test, 0, sizeof(ScgState), sm));
-    CK(cudaStreamSynchronize(sm));
-
-    // capture one outer iteration (s SpMVs, Gram + solves, update) into a graph
-    if (h->use_graph) {
-        const int64_t saved = h->launches;
-        CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
-        cudaError_t e = launch_outer(h, h->cap_stream);
-        cudaError_t e2 = cudaStreamEndCapture(h->cap_stream, &h->graph);
-        h->launches = saved;
-        if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(e));
-        CK(e2);
-        CK(cudaGraphInstantiate(&h->gexec, h->graph, 0));
-    }
+    if (int rc = setup_analyze(h)) return rc;
+    if (int rc = setup_reorder(h)) return rc;
+    if (int rc = setup_uniform_diagonal(h)) return rc;
+    if (int rc = setup_spmv_variant(h)) return rc;
+    if (int rc = setup_block_kernels(h)) return rc;
+    if (int rc = setup_mpk_wave(h)) return rc;
+    if (int rc = setup_resident(h)) return rc;
+    if (int rc = setup_workspaces(h)) return rc;
+    if (int rc = setup_graph(h)) return rc;
     h->ready = true;
     return 0;
 }
