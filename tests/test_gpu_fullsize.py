@@ -153,3 +153,39 @@ def test_config3_full_size(oracle_mod, cg_mod, torch_mod):
         if res["outer_iters"] != ref["iters"]:
             xg, _ = h.solve(bd, rtol=0.0, maxit=ref["iters"])
         assert np.linalg.norm(xg.cpu().numpy() - ref["x"]) <= 1e-8 * np.linalg.norm(ref["x"])
+
+
+@pytest.mark.parametrize("N,s", [(512, 2), (512, 8), (670, 1)])
+def test_large_index_range(cg_mod, torch_mod, N, s):
+    """Beyond every BASELINE.json config, up to the library's limit (nnz < 2^31): 7-point 512^3 (n = 134 217 728,
+    nnz = 937 951 232: byte offsets of colidx / vals beyond 2^32 and 2^33) and 670^3 (n = 300 763 000,
+    nnz = 2 102 647 600 = 0.98 * 2^31: the largest element offsets an int32 CSR can hold; 25 GB of CSR).
+    Checked against what the mathematics fixes at any size:
+    the closed-form eigenpair of the stencil (A v = lambda v, v = sin x sin x sin) through the SpMV hook
+    on every row, and after 3 outer iterations the recurrence residual the solver reports against the true residual
+    b - A x evaluated with the same hook."""
+    rp, ci, v = gen.poisson7(N)
+    n = N ** 3
+    assert rp.size - 1 == n and ci.size == 7 * N ** 3 - 6 * N ** 2 < 2 ** 31
+    t = lambda a: dev(torch_mod, a)
+    torch = torch_mod
+    g = torch.arange(1, N + 1, dtype=torch.float64, device="cuda")
+    sx = torch.sin(3 * np.pi * g / (N + 1)); sy = torch.sin(5 * np.pi * g / (N + 1)); sz = torch.sin(2 * np.pi * g / (N + 1))
+    vec = (sz[:, None, None] * sy[None, :, None] * sx[None, None, :]).reshape(-1).contiguous()     # x fastest
+    lam = 6.0 - 2.0 * (np.cos(3 * np.pi / (N + 1)) + np.cos(5 * np.pi / (N + 1)) + np.cos(2 * np.pi / (N + 1)))
+    with cg_mod.SStepCG(0) as h:
+        h.setup(t(rp), t(ci), t(v), s)
+        del rp, ci, v
+        assert h.get_info("spmv_bulk") == 1 and h.get_info("reordered") == 0 and h.get_info("resident") == 0
+        y, yj = h.test_spmv(vec)
+        assert float((y - lam * vec).abs().max()) <= 1e-13 * 12.0
+        assert float((yj - (lam / 6.0) * vec).abs().max()) <= 1e-13 * 2.0
+        del y, yj
+        b = torch.rand(n, dtype=torch.float64, device="cuda", generator=torch.Generator(device="cuda").manual_seed(5)) * 2 - 1
+        h.solve_begin(b, None, 0.0)
+        h.iterate(3)
+        x, res = h.solve_end()
+        assert res["outer_iters"] == 3 and res["status"] == 1 and 0 < res["relres"] < 1
+        ax, _ = h.test_spmv(x, jacobi=False)
+        true = float(torch.linalg.norm(b - ax) / torch.linalg.norm(b))
+        assert abs(true - res["relres"]) <= (1e-10 if s <= 4 else 1e-7) * true     # (s = 8: TMA-staged Gram / update kernels)
