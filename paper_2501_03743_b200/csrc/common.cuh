@@ -43,17 +43,27 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-// Fixed-order sum of p[0 .. cnt) by one warp (cross-block finishes): lane-strided with four independent accumulators
-// so that the L2 loads overlap; the order depends only on cnt, so the result is reproducible run to run.
+// Fixed-order sum of p[0 .. cnt) by one warp (cross-block finishes): lane-strided with eight independent accumulators,
+// the eight loads of a pass issued together so that their L2 round trips overlap (a few hundred partials cost two
+// round trips instead of five); the order depends only on cnt, so the result is reproducible run to run.
 __device__ __forceinline__ double warp_sum_array(const double* p, int cnt, int lane) {
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     int b = lane;
-    for (; b + 96 < cnt; b += 128) {
-        const double v0 = __ldcg(p + b), v1 = __ldcg(p + b + 32), v2 = __ldcg(p + b + 64), v3 = __ldcg(p + b + 96);
-        a0 += v0; a1 += v1; a2 += v2; a3 += v3;
+    for (; b + 224 < cnt; b += 256) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; k++) v[k] = __ldcg(p + b + 32 * k);
+#pragma unroll
+        for (int k = 0; k < 8; k++) a[k] += v[k];
     }
-    for (; b < cnt; b += 32) a0 += __ldcg(p + b);
-    double v = (a0 + a1) + (a2 + a3);
+    {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; k++) v[k] = (b + 32 * k < cnt) ? __ldcg(p + b + 32 * k) : 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; k++) a[k] += v[k];
+    }
+    double v = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
