@@ -195,6 +195,24 @@ def time_outer_iterations(torch, h, b, s, k_steps, warmup, barrier):
     return ms, launches, res
 
 
+def per_iteration_stats(torch, h, b, s, k_steps):
+    """Median / min / max device time of single outer iterations (an event between consecutive graph replays), in a
+    pass of its own so that the headline region stays one event pair ("median and min")."""
+    R = restart_every_for(s)
+    k = min(k_steps, R)
+    h.solve_begin(b, None, 0.0)
+    h.iterate(1)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(k + 1)]
+    evs[0].record()
+    for i in range(k):
+        h.iterate(1)
+        evs[i + 1].record()
+    torch.cuda.synchronize()
+    h.solve_end(want_x=False)
+    us = np.array([1e3 * evs[i].elapsed_time(evs[i + 1]) for i in range(k)])
+    return dict(iterations=int(k), median=float(np.median(us)), min=float(us.min()), max=float(us.max()))
+
+
 def run_ours(args):
     import torch
 
@@ -259,6 +277,8 @@ def run_ours(args):
             entry["kernel_frac_of_measured_peak"] = {k: v / peak for k, v in entry["kernel_gbs"].items()}
             t_all = s * k_us["spmv"] + sum(v for k, v in k_us.items() if k != "spmv")
             entry["kernel_share_of_step"] = {k: (v * (s if k == "spmv" else 1)) / t_all for k, v in k_us.items()}
+            if not form and h.get_info("resident") == 0:
+                entry["us_per_outer_stats"] = per_iteration_stats(torch, h, b, s, args.steps)
             if form:
                 moment[str(s)] = entry
                 continue
@@ -488,6 +508,7 @@ def main():
             "l2": "inputs larger than L2: one outer iteration streams %.1f GB >> 126 MB" % (mb["total"] / 1e9),
             "parallelism": "replicas only (north_star: one GPU, no sharding)" if world > 1 else "single GPU",
         },
+        "us_per_outer_stats": p.get("us_per_outer_stats"),   # single outer iterations (separate pass): median / min / max
         "gdof_iter_per_s": p["gdof_iter_per_s"],
         "achieved_gbs": p["achieved_gbs"],
         "iteration_roofline": {"bound": "hbm", "achieved": p["achieved_gbs"], "peak": ctx["peak"], "unit": "GB/s",
