@@ -239,13 +239,13 @@ def run_ours(args):
     runs = [(0, s) for s in s_list] + ([(1, s) for s in s_list] if args.moment_form else [])
     moment = {}
     for form, s in runs:
-        with cg.SStepCG(local, form=form, resident=1) as h:      # graph path: one launch per kernel, per-kernel times
+        with cg.SStepCG(local, form=form, resident=1, **args.extra) as h:      # graph path: one launch per kernel, per-kernel times
             torch.cuda.synchronize()
             t_setup = time.perf_counter()
             h.setup(rp, ci, va, s)
             torch.cuda.synchronize()
             t_setup = time.perf_counter() - t_setup
-            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid", "reordered", "cm_levels")}
+            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid", "reordered", "cm_levels", "pdl")}
             info["setup_seconds"] = t_setup      # validation, dinv, (auto) Cuthill-McKee reordering, workspaces, graph capture
             if s == s0 and form == 0:
                 with ClockSampler(local) as clk:
@@ -289,7 +289,7 @@ def run_ours(args):
     # two-reduction comparator on the same workload; one "outer iteration" = one CG iteration
     pcg = None
     if args.pcg:
-        with cg.SStepCG(local, method=1) as h:
+        with cg.SStepCG(local, method=1, **args.extra) as h:
             h.setup(rp, ci, va, 1)
             ms, launches, res = time_outer_iterations(torch, h, b, 1, args.steps, args.warmup, barrier)
             agg = aggregate_replicas(ms, args.steps, world, reduce_max)
@@ -306,7 +306,7 @@ def run_ours(args):
                             "us_per_cg_equiv_iter of the s-step entries")
     # resident path: what sstep_cg_solve runs by default when every CTA's rows fit shared memory
     resident = None
-    with cg.SStepCG(local) as h:
+    with cg.SStepCG(local, **args.extra) as h:
         h.setup(rp, ci, va, s0)
         if h.get_info("resident") == 1:
             ms, launches, res = time_outer_iterations(torch, h, b, s0, args.steps, args.warmup, barrier)
@@ -334,7 +334,7 @@ def run_e2e(args, ctx):
     rp, ci, va, b = pin(c["rowptr"]), pin(c["colidx"]), pin(c["vals"]), pin(c["b"])
     x = torch.empty(c["n"], dtype=torch.float64).pin_memory()
     best = None
-    with cg.SStepCG(ctx["local"]) as h:
+    with cg.SStepCG(ctx["local"], **args.extra) as h:
         for it in range(3):  # first pass warms allocator / graph instantiation paths; report the faster of the next two
             ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
@@ -460,7 +460,10 @@ def main():
     ap.add_argument("--no-pcg", dest="pcg", action="store_false", help="skip the Alg. 1 (PCG-HS) comparator line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",
+                    help="extra solver option for every handle of the run (sstep_cg_set_option), e.g. --opt pdl=0; repeatable")
     args = ap.parse_args()
+    args.extra = {kv.split("=", 1)[0]: int(kv.split("=", 1)[1]) for kv in args.opt}
     args.warmup = max(args.warmup, 3)
 
     if args.impl == "reference":
@@ -504,7 +507,7 @@ def main():
                          f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)") if args.config == 4 else
                         (f"config {args.config} ({ctx['c']['name']}): grid {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, x0=0, Jacobi, "
                          f"s={s}, rtol=0 (fixed iteration count)"),
-            "s": s, "grid": N, "restart_every": restart_every_for(s),
+            "s": s, "grid": N, "restart_every": restart_every_for(s), "options": args.extra, "pdl": p.get("pdl"),
             "l2": "inputs larger than L2: one outer iteration streams %.1f GB >> 126 MB" % (mb["total"] / 1e9),
             "parallelism": "replicas only (north_star: one GPU, no sharding)" if world > 1 else "single GPU",
         },

@@ -128,6 +128,12 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  in-order tiles couple every warp to the slowest one), hence not selected automatically.
  *                  "mpk_block_rows" (32 * 2^k; 0 = auto), "mpk_levels" (levels per pass) and "mpk_slack" (extra blocks
  *                  a level trails its predecessor by) override the shape.
+ *   "pdl"          1 (default) | 0.  Programmatic dependent launch: the kernels of one outer iteration (a1 x s, a2 + a3, a4)
+ *                  carry the programmatic-stream-serialization attribute, captured as programmatic edges of the graph, so
+ *                  the next kernel's blocks become resident while the current one drains (the SpMV also stages its first
+ *                  CSR tiles there); each kernel reads or writes solver data only behind `griddepcontrol.wait`, i.e. after
+ *                  its predecessor has completed -- results are bitwise those of pdl = 0.  Falls back to 0 by itself if
+ *                  the driver cannot capture such a graph (get_info "pdl" tells).
  *   "use_graph"    1 (default) | 0 launch kernels directly (debugging) */
 int sstep_cg_set_option(sstep_cg_t *handle, const char *key, int64_t value);
 int sstep_cg_get_info(sstep_cg_t *handle, const char *key, int64_t *value);

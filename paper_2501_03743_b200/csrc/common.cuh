@@ -77,6 +77,14 @@ __device__ __forceinline__ double group_sum(double v) {
 }
 
 // ---- mbarrier + 1-D bulk async copy (TMA engine, cp.async.bulk) -------------------------------------
+// ---- programmatic dependent launch (sm_90+): the kernels of one outer iteration are chained with the launch attribute
+// cudaLaunchAttributeProgrammaticStreamSerialization, so the blocks of kernel k+1 may become resident (and run whatever
+// does not depend on kernel k) while kernel k drains.  pdl_wait() returns once every prerequisite grid has completed and
+// its writes are visible -- nothing written by (or still read by) the predecessor may be touched before it; it is a
+// no-op for a launch without the attribute.  pdl_launch() lets the next kernel's blocks be scheduled.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }

@@ -98,6 +98,8 @@ gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ 
             const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve) {
     using Cfg = GramCfg<S>;
     constexpr int G = Cfg::G, NSL = Cfg::NSL, RG = Cfg::RG;
+    pdl_wait();  // (common.cuh: the predecessor in the graph may still be draining)
+    pdl_launch();
     if (st->status != SCG_RUNNING) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int q = warp % NSL;   // slice

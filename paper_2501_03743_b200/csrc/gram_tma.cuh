@@ -53,6 +53,8 @@ gram_tma_kernel(int64_t n, const double* __restrict__ R, const double* __restric
     using TC = GramTmaCfg<S>;
     constexpr int G = TC::G, NSL = TC::NSL, NWC = TC::NWC, NACC = TC::NACC, RPP = TC::RPP;
     constexpr int T = TC::T, COLS = TC::COLS, D = TC::D;
+    pdl_wait();  // (common.cuh: the predecessor in the graph may still be draining)
+    pdl_launch();
     if (st->status != SCG_RUNNING) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* slots = reinterpret_cast<double*>(smem_raw);

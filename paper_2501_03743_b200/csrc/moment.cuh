@@ -67,6 +67,8 @@ __device__ inline int warp_sw(int s, bool first, const double* vm, double* beta,
 // work.  mom: [2s][nblk] (row m = partials of mu^m, rows 1..2s-1 used); mu^0 comes from the update / init kernel.
 __global__ void __launch_bounds__(256) sw_kernel(int s, int nblk, const double* __restrict__ mom, ScgState* __restrict__ st,
                                                  int do_solve) {
+    pdl_wait();  // (common.cuh: the predecessor in the graph may still be draining)
+    pdl_launch();
     if (st->status != SCG_RUNNING) return;
     __shared__ double vm[2 * SCG_SMAX];
     __shared__ SwSmem sm;

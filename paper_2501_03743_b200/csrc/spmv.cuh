@@ -49,6 +49,8 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
                                                        double* __restrict__ yjac, const double* __restrict__ xprev, int mode,
                                                        const ScgState* __restrict__ st, double* __restrict__ mom_a,
                                                        double* __restrict__ mom_b) {
+    pdl_wait();
+    pdl_launch();
     if (st && st->status != SCG_RUNNING) return;
     double ma = 0.0, mb = 0.0;  // moment partials x^T (A x) and (D^-1 A x)^T (A x), see spmv_moment_finish
     const int g = threadIdx.x % L;
@@ -102,7 +104,7 @@ __global__ void __launch_bounds__(WPC * 32, MINB) spmv_bulk_kernel(int n, int nn
                                                              double* __restrict__ yjac, const double* __restrict__ xprev,
                                                              int mode, const ScgState* __restrict__ st, int num_tiles,
                                                              double* __restrict__ mom_a, double* __restrict__ mom_b) {
-    if (st && st->status != SCG_RUNNING) return;
+    // (the status test sits behind the ring prologue, after pdl_wait: the prologue touches only the constant CSR arrays)
     constexpr int RPT = 32 / L;
     constexpr int U = 8;  // entries per lane held in registers (rows up to 8 L entries need no remainder loop)
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -251,10 +253,20 @@ __global__ void __launch_bounds__(WPC * 32, MINB) spmv_bulk_kernel(int n, int nn
     }
     if (lane == 0 && D < my_tiles) tile_bounds(D, nb0, nb1);
     int lo_n, hi_n;  // per-row bounds of the next fragment to load (fetched one step ahead)
+    row_bounds(0, lo_n, hi_n);
+
+    // everything above read rowptr / colidx / vals only, which no kernel writes: under a programmatic dependent launch it
+    // overlaps the tail of the previous kernel.  x, xprev, st and the outputs belong to the predecessor until here.
+    pdl_wait();
+    pdl_launch();
+    if (st && st->status != SCG_RUNNING) {
+        // not running: the copies already issued into this warp's ring must land before the block may exit
+        for (int i = 0; i < D && i < my_tiles; i++) mbar_wait(&bars[i % D], 0u);
+        return;
+    }
 
     {
         SpmvFrag<U> cur;
-        row_bounds(0, lo_n, hi_n);
         for (int i = 0; i < my_tiles; i++) {
             const int lo = lo_n, hi = hi_n;
             row_bounds(i + 1, lo_n, hi_n);

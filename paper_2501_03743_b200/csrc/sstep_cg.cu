@@ -42,7 +42,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0, mpk_fused_opt = 0, mpk_block_opt = 0, mpk_levels_opt = 0, mpk_slack_opt = -1;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0, mpk_fused_opt = 0, mpk_block_opt = 0, mpk_levels_opt = 0, mpk_slack_opt = -1, pdl = 1;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -116,6 +116,24 @@ int fail(sstep_cg* h, int code, const std::string& msg) {
 using bulk_fn_t = void (*)(int, int, const int*, const int*, const double*, const double*, double*, double*,
                            const double*, int, const ScgState*, int, double*, double*);
 
+// launch of a hot-path kernel (every one of them starts with pdl_wait, common.cuh): with option pdl the launch carries
+// the programmatic-stream-serialization attribute, which stream capture turns into programmatic edges of the graph
+template <typename... Exp, typename... Act>
+cudaError_t launch_k(const sstep_cg* h, void (*kern)(Exp...), unsigned grid, unsigned block, size_t smem, cudaStream_t sm,
+                     Act&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = sm;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = h->pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<Exp>(args)...);
+}
+
 template <int L, bool MOM>
 bulk_fn_t bulk_kernel_mom(int depth) {
     switch (depth) {
@@ -139,13 +157,12 @@ template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if (h->bulk) {
-        bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr, h->bulk_cap)<<<h->spmv_grid, h->bulk_wpc * 32, bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc), sm>>>(
-            (int)h->n, (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, (int)h->num_tiles, mom_a, mom_b);
-    } else {
-        if (mom_a) spmv_vec_kernel<L, true><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
-        else spmv_vec_kernel<L, false><<<h->spmv_grid, 256, 0, sm>>>(h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+        return launch_k(h, bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr, h->bulk_cap), h->spmv_grid, h->bulk_wpc * 32,
+                        bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc), sm, (int)h->n, (int)h->nnz, h->rp, h->ci, h->va,
+                        x, y, yjac, xprev, mode, st, (int)h->num_tiles, mom_a, mom_b);
     }
-    return cudaGetLastError();
+    if (mom_a) return launch_k(h, spmv_vec_kernel<L, true>, h->spmv_grid, 256, 0, sm, h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
+    return launch_k(h, spmv_vec_kernel<L, false>, h->spmv_grid, 256, 0, sm, h->n, h->rp, h->ci, h->va, h->dinv, x, y, yjac, xprev, mode, st, mom_a, mom_b);
 }
 
 cudaError_t launch_spmv(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
@@ -233,12 +250,10 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
         return cudaSuccess;
     }
     if (h->staged && aligned16(R) && aligned16(AR) && aligned16(AP) && aligned16(r)) {
-        gram_tma_kernel<S><<<h->gram_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve,
-                                                                        (h->n + TC::T - 1) / TC::T);
-    } else {
-        gram_kernel<S><<<h->gram_grid_reg, Cfg::NW * 32, 0, sm>>>(h->n, R, AR, AP, r, h->partials, st, do_solve);
+        return launch_k(h, gram_tma_kernel<S>, h->gram_grid, TC::THREADS, TC::SMEM, sm, h->n, R, AR, AP, r, h->partials, st, do_solve,
+                        (h->n + TC::T - 1) / TC::T);
     }
-    return cudaGetLastError();
+    return launch_k(h, gram_kernel<S>, h->gram_grid_reg, Cfg::NW * 32, 0, sm, h->n, R, AR, AP, r, h->partials, st, do_solve);
 }
 
 template <int S, bool MOM>
@@ -267,12 +282,11 @@ cudaError_t update_SM(sstep_cg* h, cudaStream_t sm, bool configure, double* R, c
         return cudaSuccess;
     }
     if (h->staged && aligned16(R) && aligned16(AR) && aligned16(P) && aligned16(AP) && aligned16(x) && aligned16(r)) {
-        update_tma_kernel<S, MOM><<<h->update_grid, TC::THREADS, TC::SMEM, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
-                                                                                 h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
-    } else {
-        update_kernel<S, MOM><<<h->update_grid_reg, 256, 0, sm>>>(h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha, h->partials, st, rho_out, h->dinv_uniform);
+        return launch_k(h, update_tma_kernel<S, MOM>, h->update_grid, TC::THREADS, TC::SMEM, sm, h->n, R, AR, P, AP, x, r, h->dinv,
+                        beta, alpha, h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
     }
-    return cudaGetLastError();
+    return launch_k(h, update_kernel<S, MOM>, h->update_grid_reg, 256, 0, sm, h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
+                    h->partials, st, rho_out, h->dinv_uniform);
 }
 
 // the moment form's update also accumulates mu^0 = R_1^T r (compiled in only there)
@@ -377,8 +391,7 @@ cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, cons
 // moment form, after the MPK: fixed-order sum of the moment partials + Alg. 6 in one warp (replaces the Gram kernel)
 cudaError_t launch_sw(sstep_cg* h, cudaStream_t sm, ScgState* st, int do_solve) {
     h->launches++;
-    sw_kernel<<<1, 256, 0, sm>>>(h->s, h->spmv_grid, h->mom, st, do_solve);
-    return cudaGetLastError();
+    return launch_k(h, sw_kernel, 1, 256, 0, sm, h->s, h->spmv_grid, h->mom, st, do_solve);
 }
 
 // one iteration of Alg. 1 (method = 1; pcg.cuh): p = P, s_k = AP, u = R
@@ -796,13 +809,22 @@ int setup_workspaces(sstep_cg* h) {
 int setup_graph(sstep_cg* h) {
     if (h->use_graph) {
         const int64_t saved = h->launches;
-        CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
-        cudaError_t e = launch_outer(h, h->cap_stream);
-        cudaError_t e2 = cudaStreamEndCapture(h->cap_stream, &h->graph);
-        h->launches = saved;
-        if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(e));
-        CK(e2);
-        CK(cudaGraphInstantiate(&h->gexec, h->graph, 0));
+        for (int attempt = 0; attempt < 2; attempt++) {
+            CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+            cudaError_t e = launch_outer(h, h->cap_stream);
+            cudaError_t e2 = cudaStreamEndCapture(h->cap_stream, &h->graph);
+            h->launches = saved;
+            if (e == cudaSuccess && e2 == cudaSuccess) e2 = cudaGraphInstantiate(&h->gexec, h->graph, 0);
+            if (e == cudaSuccess && e2 == cudaSuccess) break;
+            // a driver that cannot capture / instantiate programmatic edges: once more with plain serialisation
+            if (h->graph) cudaGraphDestroy(h->graph);
+            h->graph = nullptr;
+            h->gexec = nullptr;
+            cudaGetLastError();
+            if (attempt == 0 && h->pdl) { h->pdl = 0; continue; }
+            if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+            CK(e2);
+        }
     }
     return 0;
 }
@@ -881,6 +903,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
         h->mpk_block_opt = (int)value;  // 32 * 2^k rows
     else if (k == "mpk_levels" && value >= 0 && value <= SSTEP_CG_SMAX) h->mpk_levels_opt = (int)value;
     else if (k == "mpk_slack" && value >= -1 && value <= (1 << 20)) h->mpk_slack_opt = (int)value;
+    else if (k == "pdl" && (value == 0 || value == 1)) h->pdl = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
 }
@@ -903,6 +926,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "launches") *value = h->launches;
     else if (k == "replace_every") *value = h->replace_every;
     else if (k == "method") *value = h->method;
+    else if (k == "pdl") *value = h->pdl;
     else if (k == "mpk_fused") *value = h->mpk_fused ? 1 : 0;
     else if (k == "bandwidth") *value = h->bandwidth;
     else if (k == "uniform_diagonal") *value = h->dinv_uniform > 0.0 ? 1 : 0;

@@ -140,6 +140,8 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
               ScgState* __restrict__ st, double* __restrict__ rho_out, double dinv_uniform) {
+    pdl_wait();  // (common.cuh: the predecessor in the graph may still be draining)
+    pdl_launch();
     if (st->status != SCG_RUNNING) return;
     __shared__ __align__(16) double sbeta[S * S];
     __shared__ double salpha[S];

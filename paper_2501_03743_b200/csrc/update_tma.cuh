@@ -46,6 +46,8 @@ update_tma_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ 
                   ScgState* __restrict__ st, double* __restrict__ rho_out, int64_t num_tiles) {
     using TC = UpdateTmaCfg<S>;
     constexpr int T = TC::T, COLS = TC::COLS, D = TC::D, NCW = TC::NCW;
+    pdl_wait();  // (common.cuh: the predecessor in the graph may still be draining)
+    pdl_launch();
     if (st->status != SCG_RUNNING) return;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* slots = reinterpret_cast<double*>(smem_raw);
