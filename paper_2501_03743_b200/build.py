@@ -9,7 +9,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsstepcg.so")
 SOURCES = ["sstep_cg.cu"]
-HEADERS = ["common.cuh", "spmv.cuh", "gram.cuh", "small_solve.cuh", "update.cuh", "tile_pipe.cuh", "gram_tma.cuh", "update_tma.cuh", "moment.cuh"]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh"))
 
 
 def _newest_source_mtime() -> float:

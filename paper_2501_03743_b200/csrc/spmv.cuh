@@ -91,6 +91,9 @@ __global__ void __launch_bounds__(256) spmv_vec_kernel(int64_t n, const int* __r
 // partial sum of any entries beyond U*L (long rows, summed when the fragment is loaded).  Once the fragment is in
 // registers the slot is free and the copy of the warp's tile i+D is issued into it.  (Loading the fragment of tile
 // i+1 before tile i is reduced was measured slower: it doubles the registers and halves the resident warps.)
+// Three CTAs per SM is the optimum, not a register accident: forced to 64 registers (MINB = 4: 32 warps per SM, 92 bytes
+// of spills) the same kernel takes 1790 us instead of 554 us on 320^3 and 103 us instead of 41 us on 128^3 -- four rings
+// (196 KB of shared memory) leave the unified L1 about 30 KB, and the x gathers live on L1 hits (68 % at three CTAs).
 template <int U>
 struct SpmvFrag {
     double v[U], xv[U];
