@@ -335,7 +335,13 @@ def run_e2e(args, ctx):
     x = torch.empty(c["n"], dtype=torch.float64).pin_memory()
     best = None
     with cg.SStepCG(ctx["local"], **args.extra) as h:
-        for it in range(3):  # first pass warms allocator / graph instantiation paths; report the faster of the next two
+        # first pass warms allocator / graph instantiation paths; report the fastest of the next two -- or, for solves of a
+        # few milliseconds (configs 1, 2), of as many as fit into ~0.3 s: after python-side gaps the GPU sits in a low
+        # power state and single short passes were seen anywhere between 2 and 40 ms
+        passes, spent = 0, 0.0
+        for it in range(40):
+            if it >= 3 and spent > 300.0:
+                break
             ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
@@ -345,6 +351,8 @@ def run_e2e(args, ctx):
             torch.cuda.synchronize()
             wall_ms = 1e3 * (time.perf_counter() - t0)
             cur = dict(ms=max(ev0.elapsed_time(ev1), wall_ms), res=res)
+            spent += cur["ms"]
+            passes += 1
             if it >= 1 and (best is None or cur["ms"] < best["ms"]):
                 best = cur
     k = best["res"]["outer_iters"]
@@ -363,7 +371,7 @@ def run_e2e(args, ctx):
     h2d = rp.numel() * 4 + ci.numel() * 4 + va.numel() * 8 + b.numel() * 8
     return dict(value=1e3 * best["ms"] / k, unit="us", h2d_bytes_per_step=h2d / k, d2h_bytes_per_step=x.numel() * 8 / k,
                 outer_iters=k, status=best["res"]["status_name"], relres=best["res"]["relres"], rtol=rtol, total_ms=best["ms"],
-                rel_error_vs_xstar=xerr, h2d_alone_ms=h2d_ms,
+                rel_error_vs_xstar=xerr, h2d_alone_ms=h2d_ms, passes=passes,
                 note="one sstep_cg_solve_host call: pinned host CSR+b -> device, setup (validation, dinv, reordering if "
                      f"needed, graph capture), the whole solve to rtol={rtol:g} ({k} outer iterations), x -> host; all "
                      "inside the timed region; value = total / outer iterations")
