@@ -42,6 +42,7 @@ def test_library_contains_sm100a_code_and_bulk_copy():
     sass = subprocess.run([cuobjdump, "-sass", cg.LIB], capture_output=True, text=True).stdout
     assert "UBLKCP" in sass              # cp.async.bulk (TMA engine) in the staged SpMV
     assert "DFMA" in sass                # fp64 arithmetic
+    assert "ACQBULK" in sass and "PREEXIT" in sass   # griddepcontrol.wait / .launch_dependents (option pdl)
 
 
 def test_no_gpu_fails_loudly():
