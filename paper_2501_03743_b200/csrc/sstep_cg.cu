@@ -30,7 +30,7 @@ struct Header {  // mirrors the first fields of ScgState
 // 7-point configs; the two larger tiles keep FEW lanes per row for longer rows (27-point: L = 2 -> 16 rows x 27, L = 1 ->
 // 32 rows x 27 per tile), because consecutive rows under the same lane index gather consecutive x entries.
 constexpr int BULK_CAP = 256, BULK_WPC = 8;
-constexpr int BULK_CAP2 = 512, BULK_WPC2 = 8;     // L = 2, depth 2 (27-point 160^3: 257 us; 6 warps x 2 CTAs 313 us, 4 warps x 4 CTAs 254 us per launch but 1292 vs 1235 us per outer iteration)
+constexpr int BULK_CAP2 = 512, BULK_WPC2 = 8;     // L = 2, depth 2 (27-point 160^3: 257 us; 6 warps x 2 CTAs 313 us, 4 warps x 4 CTAs 254 us per launch but 1292 vs 1235 us per outer iteration; 448-entry slots, i.e. 60 instead of 28 KB of L1: 256 us)
 constexpr int BULK_CAP1 = 1024, BULK_WPC1 = 4;    // L = 1, depth 2
 constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D * cap * 12 + (size_t)wpc * D * 8; }
 
