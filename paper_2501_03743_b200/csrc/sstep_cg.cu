@@ -30,7 +30,12 @@ struct Header {  // mirrors the first fields of ScgState
 // 7-point configs; the two larger tiles keep FEW lanes per row for longer rows (27-point: L = 2 -> 16 rows x 27, L = 1 ->
 // 32 rows x 27 per tile), because consecutive rows under the same lane index gather consecutive x entries.
 constexpr int BULK_CAP = 256, BULK_WPC = 8;
-constexpr int BULK_CAP2 = 512, BULK_WPC2 = 8;     // L = 2, depth 2 (27-point 160^3: 257 us; 6 warps x 2 CTAs 313 us, 4 warps x 4 CTAs 254 us per launch but 1292 vs 1235 us per outer iteration; 448-entry slots, i.e. 60 instead of 28 KB of L1: 256 us)
+// L = 2, depth 2 (27-point 160^3).  Bytes in flight decide: 8 warps x 2 CTAs on 512-entry slots 257 us per launch,
+// 10 warps x 2 CTAs on 448-entry slots (40 slots = 208 KB of copies in flight per SM, the most that fits) 230 us = 97 %
+// of the copy peak.  Measured on the way: 6 warps x 2 CTAs 313 us; 4 warps x 4 CTAs 254 us per launch but a slower outer
+// iteration; 8 warps on 448-entry slots (60 instead of 28 KB of L1) 256 us -- L1 is not the limit here.
+constexpr int BULK_CAP2 = 448, BULK_WPC2 = 10;    // tiles up to 445 entries (16 rows x 27)
+constexpr int BULK_CAP2B = 512, BULK_WPC2B = 8;   // tiles up to 509 entries (16 rows x 31)
 constexpr int BULK_CAP1 = 1024, BULK_WPC1 = 4;    // L = 1, depth 2
 constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D * cap * 12 + (size_t)wpc * D * 8; }
 
@@ -149,6 +154,7 @@ bulk_fn_t bulk_kernel_for(int depth, bool mom, int cap) {
     }
     if constexpr (L == 2) {
         if (cap == BULK_CAP2) return mom ? spmv_bulk_kernel<2, 2, BULK_CAP2, BULK_WPC2, true, 2> : spmv_bulk_kernel<2, 2, BULK_CAP2, BULK_WPC2, false, 2>;
+        if (cap == BULK_CAP2B) return mom ? spmv_bulk_kernel<2, 2, BULK_CAP2B, BULK_WPC2B, true, 2> : spmv_bulk_kernel<2, 2, BULK_CAP2B, BULK_WPC2B, false, 2>;
     }
     return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth);
 }
@@ -613,6 +619,7 @@ int setup_spmv_variant(sstep_cg* h) {
             int cap = 0, wpc = BULK_WPC;
             if (hs[2] + 3 <= BULK_CAP) cap = BULK_CAP;
             else if (Lb == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP2) { cap = BULK_CAP2; wpc = BULK_WPC2; }
+            else if (Lb == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP2B) { cap = BULK_CAP2B; wpc = BULK_WPC2B; }
             else if (Lb == 1 && h->spmv_variant == 2 && h->spmv_depth == 2 && hs[2] + 3 <= BULK_CAP1) { cap = BULK_CAP1; wpc = BULK_WPC1; }
             if (cap) {
                 h->bulk = true;
@@ -915,6 +922,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "spmv_bulk") *value = h->bulk ? 1 : 0;
     else if (k == "spmv_grid") *value = h->spmv_grid;
     else if (k == "spmv_depth") *value = h->spmv_depth;
+    else if (k == "bulk_cap") *value = h->bulk ? h->bulk_cap : 0;
     else if (k == "block_staged") *value = h->staged ? 1 : 0;
     else if (k == "form") *value = h->form;
     else if (k == "gram_grid") *value = h->gram_grid;
