@@ -135,7 +135,10 @@ __device__ __forceinline__ void update_block_finish(double rho, double mu0, int 
 }
 
 template <int S, bool MOM>
-__global__ void __launch_bounds__(256, (S <= 2) ? 4 : 2)
+// Occupancy: three CTAs per SM for s = 3, 4 (80 registers, no spills): 768 rows x 144 bytes of loads in flight per SM
+// instead of 512 -- update<4> on 320^3 1221 -> 1165 us (6.5 TB/s, the copy peak); larger s (hooks on misaligned buffers
+// only -- the staged kernel serves s >= 5) keep two.
+__global__ void __launch_bounds__(256, (S <= 2) ? 4 : (S <= 4) ? 3 : 2)
 update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
