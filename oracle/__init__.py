@@ -30,14 +30,36 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_LIB_OMP = os.path.join(_HERE, "liboracle_omp.so")
+
+
+def build_omp(force: bool = False) -> str:
+    """The same source once more with -fopenmp: the all-core timing leg of bench.py's cpu_baseline (never used for
+    parity -- its inner products are summed in another order)."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                               "-o", _LIB_OMP, _SRC, "-lm"])
+    return _LIB_OMP
+
+
 _lib = None
+_lib_omp = None
 
 
-def lib():
-    global _lib
+def lib(omp: bool = False):
+    global _lib, _lib_omp
+    if omp:
+        if _lib_omp is None:
+            _lib_omp = C.CDLL(build_omp())
+        return _lib_omp
     if _lib is None:
         _lib = C.CDLL(build())
     return _lib
+
+
+def omp_threads() -> int:
+    """Threads the OpenMP build will use (OMP_NUM_THREADS or all cores this process may run on)."""
+    return int(lib(omp=True).omp_get_max_threads())
 
 
 def _p(a, ty=C.c_double):
@@ -181,6 +203,26 @@ def pcg(rowptr, colidx, vals, b, x0=None, rtol=1e-8, maxit=2000, history=False, 
 def pfcg(rowptr, colidx, vals, b, x0=None, rtol=1e-8, maxit=2000, history=False, xhist_cap=0):
     """Alg. 2 PFCG-NN with B = diag(A)."""
     return _solver_common(lib().orc_pfcg, rowptr, colidx, vals, b, x0, rtol, maxit, (), history, xhist_cap)
+
+
+def sstep_timed(rowptr, colidx, vals, b, s, iters, omp=False, basis=0):
+    """bench.py's cpu_baseline: `iters` outer iterations of orc_sstep (Gram form, rtol = 0) with the wall clock taken
+    inside the C loop; returns (seconds per outer iteration without the start-up, start-up seconds, result dict).
+    omp = True runs the -fopenmp build of the same source on all host cores."""
+    import time
+    L = lib(omp)
+    tlog = np.zeros(iters + 1)
+    L.orc_set_time_log(_p(tlog), C.c_int(iters + 1))
+    t0 = time.perf_counter()
+    try:
+        out = _solver_common(L.orc_sstep, rowptr, colidx, vals, b, None, 0.0, iters, (C.c_int(s), C.c_int(0), C.c_int(basis)),
+                             False, 0)
+    finally:
+        L.orc_set_time_log(None, C.c_int(0))
+    total = time.perf_counter() - t0
+    assert out["iters"] == iters, out
+    per = (tlog[iters] - tlog[0]) / iters
+    return per, total - per * iters, out
 
 
 def sstep(rowptr, colidx, vals, b, s, x0=None, rtol=1e-8, maxit=2000, form="gram", basis=0,

@@ -1,7 +1,7 @@
 /*
  * oracle/sstep_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
  *
- * Plain, slow, single-threaded, obviously-correct CPU (fp64) implementation of
+ * Plain, slow, single-threaded (see ORC_PAR_FOR below for the one exception), obviously-correct CPU (fp64) implementation of
  * what the s-step PCG hot path of arxiv 2501.03743 computes, written from
  * /root/reference/PAPER.md only.  It shares no code, header, table or helper
  * with the CUDA library in paper_2501_03743_b200/; only tests/,
@@ -27,15 +27,44 @@
  * Hilbert inverse, CG <-> s-step iterate identity, A-conjugacy, the classical
  * CG error bound, the paper's 514 iterations, scipy cross-checks).
  */
+#define _POSIX_C_SOURCE 199309L /* clock_gettime under -std=c11 (timing instrumentation only) */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 
 typedef int32_t i32;
 typedef int64_t i64;
 
 #define ORC_SMAX 16
+
+/* All-core timing leg (SURVEY.md 8(d) "Oracle timed beside it", leg 2): the SAME source built a second time with
+ * -fopenmp (liboracle_omp.so) runs its row loops and inner products on all host cores.  Without the flag -- the
+ * build every pin and every parity test uses -- the two macros below expand to nothing and this file is the
+ * single-threaded program it always was, statement for statement.  (With the flag the inner products are summed
+ * per thread and then combined, i.e. in another order: that build is for bench.py's cpu_baseline only.) */
+#ifdef _OPENMP
+#define ORC_PRAGMA(x) _Pragma(#x)
+#define ORC_PAR_FOR ORC_PRAGMA(omp parallel for schedule(static))
+#define ORC_PAR_SUM(v) ORC_PRAGMA(omp parallel for schedule(static) reduction(+ : v))
+#else
+#define ORC_PAR_FOR
+#define ORC_PAR_SUM(v)
+#endif
+
+/* Timing instrumentation for bench.py (no arithmetic): if a log is set, orc_sstep_rr stores the wall clock at the
+ * start of its outer loop in tlog[0] and after outer iteration k in tlog[k + 1], so that a caller can time outer
+ * iterations without the solver's start-up (dinv, r0). */
+static double *orc_tlog = NULL;
+static int orc_tlog_cap = 0;
+void orc_set_time_log(double *tlog, int cap) { orc_tlog = tlog; orc_tlog_cap = cap; }
+static double orc_now(void)
+{
+    struct timespec ts;
+    clock_gettime(CLOCK_MONOTONIC, &ts);
+    return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
 
 /* ---------------------------------------------------------------- basics */
 
@@ -43,6 +72,7 @@ typedef int64_t i64;
 void orc_spmv(i64 n, const i32 *rowptr, const i32 *colidx, const double *vals,
               const double *x, double *y)
 {
+    ORC_PAR_FOR
     for (i64 i = 0; i < n; i++) {
         double acc = 0.0;
         for (i64 k = rowptr[i]; k < rowptr[i + 1]; k++)
@@ -68,6 +98,7 @@ int orc_dinv(i64 n, const i32 *rowptr, const i32 *colidx, const double *vals, do
 static long double ldot(i64 n, const double *a, const double *b)
 {
     long double acc = 0.0L;
+    ORC_PAR_SUM(acc)
     for (i64 i = 0; i < n; i++) acc += (long double)a[i] * (long double)b[i];
     return acc;
 }
@@ -88,6 +119,7 @@ double orc_dot(i64 n, const double *a, const double *b) { return (double)ldot(n,
 void orc_mpk(i64 n, const i32 *rowptr, const i32 *colidx, const double *vals,
              const double *dinv, const double *r, int s, int basis, double *R, double *AR)
 {
+    ORC_PAR_FOR
     for (i64 i = 0; i < n; i++) R[i] = dinv[i] * r[i];
     for (int j = 0; j < s; j++) {
         const double *Rj = R + (i64)j * n;
@@ -96,11 +128,14 @@ void orc_mpk(i64 n, const i32 *rowptr, const i32 *colidx, const double *vals,
         if (j + 1 < s) {
             double *Rn = R + (i64)(j + 1) * n;
             if (basis == 0) {
+                ORC_PAR_FOR
                 for (i64 i = 0; i < n; i++) Rn[i] = dinv[i] * ARj[i];
             } else if (j == 0) {
+                ORC_PAR_FOR
                 for (i64 i = 0; i < n; i++) Rn[i] = dinv[i] * ARj[i] - Rj[i];
             } else {
                 const double *Rp = R + (i64)(j - 1) * n;
+                ORC_PAR_FOR
                 for (i64 i = 0; i < n; i++) Rn[i] = 2.0 * (dinv[i] * ARj[i] - Rj[i]) - Rp[i];
             }
         }
@@ -271,8 +306,9 @@ int orc_sw(int s, const double *vm, double *alpha, double *beta, double *W)
 void orc_update(i64 n, int s, const double *R, const double *AR, double *P, double *AP,
                 double *x, double *r, const double *beta, const double *alpha)
 {
-    double pn[ORC_SMAX], apn[ORC_SMAX];
+    ORC_PAR_FOR
     for (i64 i = 0; i < n; i++) {
+        double pn[ORC_SMAX], apn[ORC_SMAX];
         for (int j = 0; j < s; j++) {
             double p = R[(i64)j * n + i], ap = AR[(i64)j * n + i];
             for (int l = 0; l < s; l++) {
@@ -424,6 +460,7 @@ int orc_sstep_rr(i64 n, const i32 *rp, const i32 *ci, const double *v, const dou
     double nr0 = sqrt((double)ldot(n, r, r));
     *relres = 1.0;
     if (nr0 == 0.0) { status = 0; *relres = 0.0; goto done; }
+    if (orc_tlog && orc_tlog_cap > 0) orc_tlog[0] = orc_now();
     for (int k = 0; k < maxit; k++) {                                  /* l.3 */
         orc_mpk(n, rp, ci, v, dinv, r, s, basis, R, AR);               /* l.5 / l.23 */
         int st;
@@ -452,6 +489,7 @@ int orc_sstep_rr(i64 n, const i32 *rp, const i32 *ci, const double *v, const dou
         *relres = nr / nr0;
         if (hist) hist[k] = *relres;
         if (xhist && k < xhist_cap) memcpy(xhist + (i64)k * n, x, sizeof(double) * n);
+        if (orc_tlog && k + 1 < orc_tlog_cap) orc_tlog[k + 1] = orc_now();
         if (!isfinite(nr)) { status = 2; break; }
         if (nr < rtol * nr0) { status = 0; break; }                    /* l.31-33 */
         if (replace_every > 0 && (k + 1) % replace_every == 0) {
