@@ -75,13 +75,22 @@ def ncu_traffic(config: int, s: int, prefix: str = "spmv"):
         return None
 
 
+def workload_string(config: int, N: int, n: int, nnz: int, s: int, name: str = "") -> str:
+    """config.workload -- the SAME string in both arms (ours / --impl reference), so the driver can tell they ran the same job."""
+    if config == 4:
+        return (f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, b=A x*, x*~U[-1,1] seed 3, "
+                f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)")
+    return (f"config {config} ({name}): grid {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, x0=0, Jacobi, "
+            f"s={s}, rtol=0 (fixed iteration count)")
+
+
 def restart_every_for(s: int) -> int:
     return max(1, 100 // s)       # <= 100 CG-equivalent steps per restart: far from convergence at 320^3
 
 
 # ----------------------------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms from before the warm-up to the end of the timed region."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -96,8 +105,12 @@ class ClockSampler:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
             os.close(fd)
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "200", "-i", str(self.idx)], stdout=open(self.path, "w"),
+                                          "-lms", "20", "-i", str(self.idx)], stdout=open(self.path, "w"),
                                          stderr=subprocess.DEVNULL)
+            for _ in range(100):                 # nvidia-smi takes a moment to start: wait for its first sample
+                if os.path.getsize(self.path) > 0:
+                    break
+                time.sleep(0.02)
         except Exception:
             self.proc = None
         return self
@@ -114,12 +127,18 @@ class ClockSampler:
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         try:
             rows = [ln.split(",") for ln in open(self.path).read().strip().splitlines() if ln.strip()]
+            rows = [r for r in rows if len(r) >= 9]          # (a sample cut off by terminate())
             sm = [float(r[1]) for r in rows]
             out["samples"] = len(sm)
             if sm:
-                out["sm_mhz"] = float(np.median(sm))
+                pw = np.array([float(r[3]) for r in rows])
+                load = pw >= 0.5 * (pw.min() + pw.max())   # samples taken while the kernels ran (power well above idle)
+                out["samples_under_load"] = int(load.sum())
+                out["sm_mhz"] = float(np.median(np.array(sm)[load])) if load.any() else float(np.median(sm))
+                out["sm_mhz_min"] = float(np.min(np.array(sm)[load])) if load.any() else float(np.min(sm))
                 out["sm_max_mhz"] = float(rows[0][2])
-                out["power_w_max"] = max(float(r[3]) for r in rows)
+                out["power_w_max"] = float(pw.max())
+                out["sample_period_ms"] = 20
             names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
             for j, nm in enumerate(names):
                 if any(r[5 + j].strip().lower().startswith("active") for r in rows):
@@ -235,6 +254,8 @@ def run_ours(args):
 
     sweep = {}
     primary = None
+    sustained = None
+    read_peak = None
     s_list = [s0] + [int(t) for t in args.sweep.split(",") if t and int(t) != s0] if args.sweep else [s0]
     runs = [(0, s) for s in s_list] + ([(1, s) for s in s_list] if args.moment_form else [])
     moment = {}
@@ -251,6 +272,28 @@ def run_ours(args):
                 with ClockSampler(local) as clk:
                     ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)
                 clocks = clk.summary()
+                # sustained: the same step for >= 2 s (the headline region of a short --steps run is a burst at boost clocks;
+                # a long solve runs under the power cap), its own clock samples beside it
+                if args.sustained_s > 0:
+                    R = restart_every_for(s)
+                    k_sus = int(np.ceil(args.sustained_s * 1e3 / (ms / args.steps) / R)) * R
+                    with ClockSampler(local) as clk2:
+                        ms2, _, _ = time_outer_iterations(torch, h, b, s, k_sus, args.warmup, barrier)
+                    us2 = 1e3 * reduce_max(ms2) / k_sus
+                    mbs = model_bytes(n, nnz, s, form)["total"]
+                    sustained = dict(us_per_outer=us2, steps=k_sus, seconds=ms2 / 1e3, achieved_gbs=mbs / (us2 * 1e-6) / 1e9,
+                                     frac_of_measured_peak=mbs / (us2 * 1e-6) / 1e9 / peak, clocks=clk2.summary())
+                # read-side and copy bandwidth of this box from the library's own streaming kernels (csrc/measure.cuh)
+                if args.read_peak:
+                    big = 8 << 30
+                    rp_ldg = h.measure_bandwidth(0, big, 1, 5)
+                    rp_bulk = max(h.measure_bandwidth(1, big, 1, 5), h.measure_bandwidth(3, big, 1, 5))
+                    cp = h.measure_bandwidth(2, big // 2, 1, 5)
+                    l2 = max(h.measure_bandwidth(0, 48 << 20, 64, 5), h.measure_bandwidth(1, 48 << 20, 64, 5))
+                    read_peak = dict(read_ldg_gbs=rp_ldg[0], read_bulk_gbs=rp_bulk[0], read_peak_gbs=max(rp_ldg[0], rp_bulk[0]),
+                                     copy_gbs=cp[0], l2_read_48mb_gbs=l2[0], mean=dict(read_ldg=rp_ldg[1], read_bulk=rp_bulk[1], copy=cp[1], l2=l2[1]),
+                                     how="sstep_cg_measure_bandwidth: 8 GiB zero-filled buffer read once per launch (copy: 4 GiB "
+                                         "read + 4 GiB written), best / mean of 5 launches; l2 = a 48 MiB buffer read 64 times in one launch")
             else:
                 ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)
             agg = aggregate_replicas(ms, args.steps, world, reduce_max)
@@ -316,7 +359,7 @@ def run_ours(args):
                             gdof_iter_per_s=world * n * s0 / (1e3 * agg["ms_per_step"] * 1e-6) / 1e9, relres_at_end=res["relres"],
                             note="whole loop in one cooperative launch per restart (csrc/resident.cuh); s + 1 grid barriers per outer iteration")
     return dict(world=world, rank=rank, local=local, c=c, n=n, nnz=nnz, N=N, sweep=sweep, moment=moment, primary=primary, clocks=clocks,
-                resident=resident, pcg=pcg,
+                resident=resident, pcg=pcg, sustained=sustained, read_peak=read_peak,
                 peak=peak, peak_src=peak_src, t_gen=t_gen, dev=(rp, ci, va, b))
 
 
@@ -378,25 +421,38 @@ def run_e2e(args, ctx):
 
 
 def run_cpu_baseline(args, ctx):
-    """The oracle as it stands, on the host cores of this box, on a bounded sample of the same workload."""
+    """The oracle as it stands, on the host cores of this box, on a bounded sample of the same workload: `iters` outer
+    iterations at full size, clocked inside the C loop (start-up excluded), (1) single-threaded as written and (2) the
+    same source built with -fopenmp on all cores this process may use (SURVEY.md 8(d) "Oracle timed beside it")."""
     import oracle
     c, s = ctx["c"], args.s
-    iters = 2
-    t0 = time.perf_counter()
-    ref = oracle.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=0.0, maxit=iters)
-    dt = time.perf_counter() - t0
-    assert ref["iters"] == iters
-    return dict(value=1e6 * dt / iters, unit="us", cores=1, kind="oracle",
-                sample=f"first {iters} outer iterations (s={s}) of the same {ctx['N']}^3 system at full size, single thread, "
-                       f"including the oracle's own start-up (dinv, r0)", seconds=dt)
+    iters = args.cpu_iters
+    mb = model_bytes(ctx["n"], ctx["nnz"], s)["total"]
+    cores = len(os.sched_getaffinity(0))
+    per_omp, start_omp, _ = oracle.sstep_timed(c["rowptr"], c["colidx"], c["vals"], c["b"], s, iters, omp=True)
+    per_1, start_1, _ = oracle.sstep_timed(c["rowptr"], c["colidx"], c["vals"], c["b"], s, iters, omp=False)
+    threads = oracle.omp_threads()
+    leg = lambda per: dict(us_per_outer=1e6 * per, gdof_iter_per_s=ctx["n"] * s / per / 1e9, effective_gbs=mb / per / 1e9)
+    # (value = the all-core leg; should a box's CPU quota make it the slower one, the single-thread leg is reported instead)
+    best_is_omp = per_omp <= per_1
+    return dict(value=1e6 * (per_omp if best_is_omp else per_1), unit="us", cores=threads if best_is_omp else 1, kind="oracle",
+                value_leg="all_cores" if best_is_omp else "single_thread",
+                sample=f"{iters} outer iterations (s={s}) of the same {ctx['N']}^3 system at full size, the oracle's start-up "
+                       f"(dinv, r0) excluded; value = oracle/sstep_oracle.c built with -fopenmp on {threads} threads "
+                       f"(sched_getaffinity: {cores} cores), single_thread = the same file as the parity tests use it",
+                all_cores=leg(per_omp), single_thread=dict(leg(per_1), cores=1), iterations=iters,
+                startup_seconds=dict(all_cores=start_omp, single_thread=start_1),
+                note="a reported baseline, not the target: a deliberately plain program (long double inner products)")
 
 
 # ----------------------------------------------------------------------------------------------- reference arm
 def run_reference(args):
-    """--impl reference: the oracle (oracle/sstep_oracle.c, as it stands, single thread) on this box's host cores.
+    """--impl reference: the oracle (oracle/sstep_oracle.c, as it stands) on this box's host cores.
     A step is ONE oracle outer iteration on a bounded sample of config 4: the 7-point operator on a
-    grid x grid x nz z-slab (same plane size, same nnz/row), nz sized so that warm-up + K steps end within
-    ~2.5 minutes; the reported value is scaled by grid/nz to the rows of the full workload."""
+    grid x grid x nz z-slab (same plane size, same nnz/row; nz = grid, i.e. the whole system, when the budget allows),
+    nz sized so that warm-up + K steps end within ~2.5 minutes; a value measured on a slab is scaled by grid/nz to the
+    rows of the full workload.  value = the -fopenmp build of the same source on all cores; the single-threaded build
+    (the one the parity tests use) is timed beside it on the same slab for a few iterations."""
     import oracle
     world, rank, _ = dist_env()
     if rank != 0:
@@ -405,44 +461,57 @@ def run_reference(args):
     R = restart_every_for(s)
 
     def slab(nz):
+        if nz == N:                          # the full workload itself
+            c = gen.make_config(4, N=N)
+            return c["rowptr"], c["colidx"], c["vals"], c["b"]
         rp, ci, va = gen.poisson7_box(N, N, nz)
         xs = np.random.default_rng(3).uniform(-1.0, 1.0, N * N * nz)
         return rp, ci, va, gen.apply_poisson7_box(N, N, nz, xs)
 
     rp, ci, va, b = slab(4)
-    t0 = time.perf_counter()
-    oracle.sstep(rp, ci, va, b, s, rtol=0.0, maxit=2)
-    per_row = (time.perf_counter() - t0) / 2 / (N * N * 4)
-    budget = float(os.environ.get("SSTEP_REF_BUDGET_S", "150"))
+    per_row = oracle.sstep_timed(rp, ci, va, b, s, 2, omp=True)[0] / (N * N * 4)
+    budget = float(os.environ.get("SSTEP_REF_BUDGET_S", "120"))
     nz = int(max(2, min(N, budget / ((K + W) * per_row * N * N))))
     rp, ci, va, b = slab(nz)
 
-    def run(k):
+    def run(k, omp):
         done, t = 0, 0.0
         while done < k:
             kk = min(R, k - done)
-            t0 = time.perf_counter()
-            res = oracle.sstep(rp, ci, va, b, s, rtol=0.0, maxit=kk)
-            t += time.perf_counter() - t0
+            per, _, res = oracle.sstep_timed(rp, ci, va, b, s, kk, omp=omp)
             assert res["iters"] == kk and res["status"] == 1, res
+            t += per * kk
             done += kk
         return t
 
-    run(W)
-    t = run(K)
-    us_sample = 1e6 * t / K
+    run(W, True)
+    t = run(K, True)
+    k1 = max(1, min(K, 3))
+    t1 = run(k1, False)
+    threads, cores = oracle.omp_threads(), len(os.sched_getaffinity(0))
+    us_full_1 = 1e6 * t1 / k1 * N / nz
+    value_leg = "all_cores"
+    if t1 / k1 < t / K:      # a CPU quota below the visible core count: the single-thread leg is the better baseline
+        t, K_eff, threads_used, value_leg = t1, k1, 1, "single_thread"
+    else:
+        K_eff, threads_used = K, threads
+    us_sample = 1e6 * t / K_eff
     us_full = us_sample * N / nz
     n, nnz = N ** 3, 7 * N ** 3 - 6 * N ** 2
-    sample = (f"{K} oracle outer iterations (s={s}) on the {N}x{N}x{nz} z-slab of the {N}^3 7-point system, single thread, "
-              f"restarted from x0=0 every {R} iterations; value scaled by {N}/{nz} to the full row count")
+    mb = model_bytes(n, nnz, s)["total"]
+    sample = (f"{K} oracle outer iterations (s={s}) on the {N}x{N}x{nz} z-slab of the {N}^3 7-point system"
+              + (" (the whole system)" if nz == N else f"; value scaled by {N}/{nz} to the full row count")
+              + f", oracle/sstep_oracle.c built with -fopenmp on {threads} threads (sched_getaffinity: {cores} cores), start-up "
+              f"excluded, restarted from x0=0 every {R} iterations; single_thread = the plain build, {k1} iterations on the same slab; "
+              f"value = the {value_leg} leg")
     return {
         "metric": METRIC, "value": us_full, "unit": "us", "n_gpus": args.gpus, "steps": K, "warmup": W,
         "ms_per_step": us_full / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "impl": "reference",
-        "config": {"workload": f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, Jacobi, s={s}",
-                   "s": s, "sample": sample},
-        "cpu_baseline": {"value": us_full, "unit": "us", "cores": 1, "kind": "oracle", "sample": sample,
-                         "measured_us_per_step_on_sample": us_sample},
+        "config": {"workload": workload_string(4, N, n, nnz, s), "s": s, "grid": N, "restart_every": R, "sample": sample},
+        "cpu_baseline": {"value": us_full, "unit": "us", "cores": threads_used, "kind": "oracle", "sample": sample, "value_leg": value_leg,
+                         "measured_us_per_step_on_sample": us_sample, "effective_gbs": mb / (us_full * 1e-6) / 1e9,
+                         "single_thread": {"us_per_outer": us_full_1, "cores": 1, "effective_gbs": mb / (us_full_1 * 1e-6) / 1e9}},
         "e2e": {"value": us_full, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
         "gdof_iter_per_s": n * s / (us_full * 1e-6) / 1e9,
@@ -466,7 +535,10 @@ def main():
     ap.add_argument("--no-moment-form", dest="moment_form", action="store_false",
                     help="skip the extra lines for the moment form (option form = 1) of the same block sizes")
     ap.add_argument("--no-pcg", dest="pcg", action="store_false", help="skip the Alg. 1 (PCG-HS) comparator line")
+    ap.add_argument("--sustained-s", type=float, default=2.0, help="length in seconds of the extra sustained pass (0 = skip)")
+    ap.add_argument("--no-read-peak", dest="read_peak", action="store_false", help="skip the read-side / copy / L2 bandwidth probes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-iters", type=int, default=5, help="oracle outer iterations timed per cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",
                     help="extra solver option for every handle of the run (sstep_cg_set_option), e.g. --opt pdl=0; repeatable")
@@ -511,10 +583,7 @@ def main():
         "dtype": "f64",
         "data": "synthetic",
         "config": {
-            "workload": (f"config 4: 3-D Poisson 7-point {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, b=A x*, x*~U[-1,1] seed 3, "
-                         f"x0=0, Jacobi, s={s}, rtol=0 (fixed iteration count)") if args.config == 4 else
-                        (f"config {args.config} ({ctx['c']['name']}): grid {N}^3 (n={n}, nnz={nnz}), CSR fp64/int32, x0=0, Jacobi, "
-                         f"s={s}, rtol=0 (fixed iteration count)"),
+            "workload": workload_string(args.config, N, n, nnz, s, ctx["c"]["name"]),
             "s": s, "grid": N, "restart_every": restart_every_for(s), "options": args.extra, "pdl": p.get("pdl"),
             "l2": "inputs larger than L2: one outer iteration streams %.1f GB >> 126 MB" % (mb["total"] / 1e9),
             "parallelism": "replicas only (north_star: one GPU, no sharding)" if world > 1 else "single GPU",
@@ -534,7 +603,12 @@ def main():
                      "traffic": ncu_traffic(args.config, s) if N == c_default_grid(args.config) else None,
                      "traffic_source": "profiles/ncu_traffic.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)"},
         "kernels": {"us": p["kernel_us"], "gbs": p["kernel_gbs"], "frac_of_measured_peak": p["kernel_frac_of_measured_peak"],
-                    "share_of_step": p["kernel_share_of_step"]},
+                    "share_of_step": p["kernel_share_of_step"],
+                    # the SpMV is 87 % reads and the Gram kernel 99.9 %: against the READ-side wall of this box
+                    "frac_of_read_peak": ({k: p["kernel_gbs"][k] / ctx["read_peak"]["read_peak_gbs"] for k in ("spmv", "gram")
+                                           if k in p["kernel_gbs"]} if ctx["read_peak"] else None)},
+        "read_peak": ctx["read_peak"],
+        "sustained": ctx["sustained"],
         "sweep": ctx["sweep"],
         "pcg_hs": ctx["pcg"],             # Alg. 1 as its own kernel sequence (comparator, not the headline)
         "resident_path": ctx["resident"],  # only for problems that fit shared memory (config 1), else null

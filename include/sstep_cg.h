@@ -25,7 +25,8 @@
  *     int32 indices.  All work is enqueued on the stream given at create();
  *     functions that return results to the host synchronise that stream.
  *   - CSR: 0-based, rowptr[n+1], colidx[nnz], vals[nnz]; every row holds its
- *     diagonal entry and it is > 0.  Column order inside a row is free.
+ *     diagonal entry exactly once and it is > 0 (checked at setup).  Column order inside a
+ *     row is free; other duplicated (row, column) entries are summed.
  *     The three arrays are BORROWED: the caller keeps them alive and unchanged
  *     until sstep_cg_destroy or the next sstep_cg_setup.
  *   - n x s blocks in the test hooks use two layouts:
@@ -49,7 +50,11 @@ extern "C" {
 /* solver outcomes (return value of solve / field status) */
 #define SSTEP_CG_CONVERGED 0       /* ||r|| < rtol ||r0||                                   */
 #define SSTEP_CG_MAXIT 1           /* "did not converge within kmax iterations"; x valid */
-#define SSTEP_CG_BREAKDOWN 2       /* non-positive / non-finite Cholesky pivot or NaN; x = last good iterate */
+#define SSTEP_CG_BREAKDOWN 2       /* numerical breakdown.  Non-positive / non-finite Cholesky pivot or non-finite alpha
+                                    * (detected BEFORE the block update, which is then skipped): x = the last good
+                                    * iterate.  Non-finite ||r||^2 after a block update (overflow inside it): x, r, P, AP
+                                    * already hold that update and may be non-finite -- restart from your own x0. */
+#define SSTEP_CG_RUNNING (-1)      /* only in sstep_cg_solve_peek's out->status: the stop test has not fired yet */
 /* errors */
 #define SSTEP_CG_ERR_ARG (-1)
 #define SSTEP_CG_ERR_CUDA (-2)
@@ -87,7 +92,10 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
 
 /* Options, to be set between create and setup (unknown key -> ERR_ARG):
  *   "basis"        0 monomial (default) | 1 chebyshev
- *   "spmv_variant" 0 auto (default) | 1 force the generic vector-per-row kernel | 2 force the bulk-staged kernel
+ *   "spmv_variant" 0 auto (default) | 1 force the generic vector-per-row kernel | 2 force the bulk-staged kernel with
+ *                  per-warp rings | 3 force the CTA-pipelined bulk-staged kernel (thread-per-row matrices; auto picks it
+ *                  there: few large bulk copies in flight per SM instead of many small ones)
+ *   "spmv_cta_depth" 2 | 3 (default) | 4 stages of the CTA-pipelined SpMV's ring; "spmv_cta_per_sm" 2 | 3 (default) CTAs per SM
  *   "lanes"        0 auto | 1,2,4,8,16,32 lanes per row
  *   "spmv_depth"   2 (default) | 3 | 4 slots of the bulk-staged SpMV's per-warp shared-memory ring
  *   "block_variant" 0 auto (default: Gram/update through the TMA tile pipeline for s >= 5, register kernels below)
@@ -119,15 +127,18 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  stop test, direction update): the classical two-reduction comparator.  Needs s = 1 at setup;
  *                  "outer iterations" are then CG iterations.  (The paper's one-reduction baseline "fcg", Alg. 2, is
  *                  method 0 with s = 1.)
- *   "mpk_fused"    0 / 1 off (default) | 2 on (EXPERIMENTAL).  Wavefront-ordered matrix-powers kernel (csrc/mpk_wave.cuh):
- *                  the s SpMVs of Alg. 4 run as ONE kernel whose levels follow each other down a banded matrix a few row
- *                  blocks apart, so that the CSR arrays (and the basis vectors) are re-read from L2 instead of HBM.
- *                  Applies to thread-per-row matrices on the bulk-staged SpMV (7-point configs) with s >= 2, form = 0,
- *                  n % 4 == 0; bitwise the same results as the separate SpMVs.  Measured on 320^3: DRAM reads per two
- *                  levels 3.2 -> 1.6 GB as designed, but 820 us per level against 550 us (the statically assigned,
- *                  in-order tiles couple every warp to the slowest one), hence not selected automatically.
- *                  "mpk_block_rows" (32 * 2^k; 0 = auto), "mpk_levels" (levels per pass) and "mpk_slack" (extra blocks
- *                  a level trails its predecessor by) override the shape.
+ *   "mpk_fused"    0 auto | 1 off | 2 force.  Wavefront-ordered matrix-powers kernel (csrc/mpk_wave.cuh): the s SpMVs of
+ *                  Alg. 4 run as ONE kernel per pass of g levels whose levels follow each other down a banded matrix a
+ *                  fixed distance apart, so that the CSR arrays (and the basis vectors) are re-read from L2 instead of
+ *                  HBM: persistent CTAs claim work items (level, block of 512 rows) in wavefront order with one atomic
+ *                  each; per-item done flags + per-level watermarks carry the dependencies.  Applies to thread-per-row
+ *                  matrices on the CTA-pipelined SpMV (7-point configs) with s >= 2, form = 0, n % 4 == 0 and 16-byte
+ *                  aligned rowptr; bitwise the same results as the separate SpMVs.  Hardware assumption (stated in the
+ *                  file header): the gathers of a column written by other SMs in the same launch go through L1 without an
+ *                  acquire -- no sector can be cached before it is final, and the writers publish with a gpu-scope release.
+ *                  "mpk_levels" (levels per pass, 0 = as many as keep the re-read window inside L2), "mpk_slack" (blocks a
+ *                  level trails its predecessor by beyond the dependency distance, -1 = auto) and "mpk_block_rows"
+ *                  (0 = 512 | 64: small items for dependency tests on small matrices) override the shape.
  *   "pdl"          1 (default) | 0.  Programmatic dependent launch: the kernels of one outer iteration (a1 x s, a2 + a3, a4)
  *                  carry the programmatic-stream-serialization attribute, captured as programmatic edges of the graph, so
  *                  the next kernel's blocks become resident while the current one drains (the SpMV also stages its first
@@ -153,6 +164,10 @@ int sstep_cg_solve(sstep_cg_t *handle, const double *b, const double *x0, double
 int sstep_cg_solve_begin(sstep_cg_t *handle, const double *b, const double *x0, double rtol);
 int sstep_cg_iterate(sstep_cg_t *handle, int k_outer);
 int sstep_cg_solve_end(sstep_cg_t *handle, double *x, sstep_cg_result *out);
+/* Between solve_begin and solve_end: synchronise the stream and report where the solve stands (outer_iters, relres of
+ * the recurrence residual after the last completed outer iteration -- the history of Alg. 3 l.31-33 when called after
+ * every sstep_cg_iterate(h, 1) -- and status = SSTEP_CG_RUNNING / CONVERGED / BREAKDOWN).  The solve goes on. */
+int sstep_cg_solve_peek(sstep_cg_t *handle, sstep_cg_result *out);
 
 /* End-to-end convenience with HOST buffers: uploads CSR, b, x0 (NULL = zeros),
  * runs setup + solve on a private device copy, downloads x.  This is the call
@@ -168,6 +183,17 @@ int sstep_cg_solve_host(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_
  * launches, ms_host[1] = of the reps Gram+solve launches, ms_host[2] = of the reps update launches.
  * Synchronises the stream.  The iterations count as real ones (x, r, k advance). */
 int sstep_cg_profile_outer(sstep_cg_t *handle, int reps, double *ms_host);
+
+/* Measurement aid (bench.py's read-side peak): stream a private zero-filled buffer of `bytes` bytes (>= 1 MiB, rounded
+ * down to 4 KiB) `passes` times inside one launch with hand-written kernels that use the hot path's own load
+ * instructions, `reps` timed launches after one warm-up (CUDA events on the solver's stream):
+ *   variant 0  128-bit ld.global.nc.L1::no_allocate reads     (Gram / update kernels' loads)
+ *   variant 1  cp.async.bulk reads, 2 x 4 KiB ring per warp   (bulk-staged SpMV's loads)
+ *   variant 3  cp.async.bulk reads, 4 x 2 KiB ring per warp
+ *   variant 2  128-bit copy; read + written bytes both counted (comparable with MEASURED_PEAKS.json hbm_gbs)
+ * gbs_out_host[0] = best, [1] = mean GB/s.  bytes >> L2 with passes = 1 gives the HBM figure; a buffer that fits L2
+ * with passes > 1 gives the L2-hit bandwidth.  Not allowed during a solve. */
+int sstep_cg_measure_bandwidth(sstep_cg_t *handle, int variant, int64_t bytes, int passes, int reps, double *gbs_out_host);
 
 int sstep_cg_destroy(sstep_cg_t *handle);
 
@@ -206,6 +232,12 @@ int sstep_cg_test_gram(sstep_cg_t *handle, const double *R_cm, const double *AR_
 /* a3: beta = -Wprev^-1 C, W = M + C^T beta, alpha = W^-1 m; status_out[0] = 0 or SSTEP_CG_BREAKDOWN. */
 int sstep_cg_test_small_solve(sstep_cg_t *handle, const double *M, const double *C, const double *m,
                               const double *Wprev, double *beta, double *alpha, double *W, int32_t *status_out);
+/* a3 as the solver loop runs it: the Cholesky factor of the previous W is carried over instead of recomputed
+ * (Lprev: s*s row-major, lower triangle, zeros above); Lout = the factor of the new W.  Same bits as the call above
+ * with Wprev = Lprev Lprev^T's source matrix, because that call computes exactly this factor first. */
+int sstep_cg_test_small_solve_carried(sstep_cg_t *handle, const double *M, const double *C, const double *m,
+                                      const double *Lprev, double *beta, double *alpha, double *W, double *Lout,
+                                      int32_t *status_out);
 /* a4, in place: P, AP (interleaved), x, r updated; R_cm(:,1) <- D^-1 r_new; rho_out[0] = ||r_new||^2. */
 int sstep_cg_test_update(sstep_cg_t *handle, double *R_cm, const double *AR_cm, double *P_il, double *AP_il,
                          double *x, double *r, const double *beta, const double *alpha, double *rho_out);

@@ -22,7 +22,8 @@ SMAX = 16
 STATUS_NAMES = {0: "converged", 1: "maxit", 2: "breakdown"}
 EXPORTED_SYMBOLS = [
     "sstep_cg_create", "sstep_cg_setup", "sstep_cg_set_option", "sstep_cg_get_info", "sstep_cg_solve",
-    "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_profile_outer", "sstep_cg_solve_host", "sstep_cg_destroy",
+    "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_solve_peek", "sstep_cg_profile_outer",
+    "sstep_cg_measure_bandwidth", "sstep_cg_test_small_solve_carried", "sstep_cg_solve_host", "sstep_cg_destroy",
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
     "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update", "sstep_cg_test_read_state",
@@ -67,7 +68,10 @@ def load_library(build: bool = True):
     lib.sstep_cg_solve_begin.argtypes = [vp, vp, vp, dbl]
     lib.sstep_cg_iterate.argtypes = [vp, i32]
     lib.sstep_cg_solve_end.argtypes = [vp, vp, C.POINTER(_Result)]
+    lib.sstep_cg_solve_peek.argtypes = [vp, C.POINTER(_Result)]
     lib.sstep_cg_profile_outer.argtypes = [vp, i32, C.POINTER(dbl)]
+    lib.sstep_cg_measure_bandwidth.argtypes = [vp, i32, i64, i32, i32, C.POINTER(dbl)]
+    lib.sstep_cg_test_small_solve_carried.argtypes = [vp] + [vp] * 9
     lib.sstep_cg_solve_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, dbl, i32, C.POINTER(_Result)]
     lib.sstep_cg_destroy.argtypes = [vp]
     lib.sstep_cg_last_error.argtypes = [vp]
@@ -179,11 +183,12 @@ class SStepCG:
         self._check(self._lib.sstep_cg_get_permutation(self._h, self._ptr(perm)), "sstep_cg_get_permutation")
         return perm
 
-    def solve(self, b, x0=None, rtol: float = 1e-8, maxit: int = 2000):
+    def solve(self, b, x0=None, rtol: float = 1e-8, maxit: int = 2000, out=None):
+        """sstep_cg_solve; `out` = the tensor that receives x (may be x0 itself: the ABI allows the alias)."""
         torch = _torch()
         b = self._dev(b, torch.float64, "b", self.n)
         x0 = self._dev(x0, torch.float64, "x0", self.n)
-        x = torch.empty_like(b)
+        x = torch.empty_like(b) if out is None else self._dev(out, torch.float64, "out", self.n)
         res = _Result()
         self._check(self._lib.sstep_cg_solve(self._h, self._ptr(b), self._ptr(x0), self._ptr(x), float(rtol), int(maxit),
                                              C.byref(res)), "sstep_cg_solve")
@@ -198,6 +203,21 @@ class SStepCG:
 
     def iterate(self, k_outer: int):
         self._check(self._lib.sstep_cg_iterate(self._h, int(k_outer)), "sstep_cg_iterate")
+
+    def solve_peek(self):
+        """Where the solve in progress stands (status -1 = still running); the solve goes on."""
+        res = _Result()
+        self._check(self._lib.sstep_cg_solve_peek(self._h, C.byref(res)), "sstep_cg_solve_peek")
+        d = res.as_dict()
+        d["status_name"] = "running" if d["status"] == -1 else d["status_name"]
+        return d
+
+    def measure_bandwidth(self, variant: int, nbytes: int, passes: int = 1, reps: int = 5):
+        """(best, mean) GB/s of the library's streaming kernels (see sstep_cg.h): 0 ldg reads, 1 / 3 bulk reads, 2 copy."""
+        out = (C.c_double * 2)()
+        self._check(self._lib.sstep_cg_measure_bandwidth(self._h, int(variant), int(nbytes), int(passes), int(reps), out),
+                    "sstep_cg_measure_bandwidth")
+        return float(out[0]), float(out[1])
 
     def profile_outer(self, reps: int):
         """Per-kernel-class device milliseconds of `reps` un-graphed outer iterations: (spmv, gram, update)."""
@@ -302,6 +322,21 @@ class SStepCG:
                                                         self._ptr(beta), self._ptr(alpha), self._ptr(W), self._ptr(st)),
                     "sstep_cg_test_small_solve")
         return int(st.item()), beta, alpha, W
+
+    def test_small_solve_carried(self, M, Cm, m, Lprev):
+        """a3 with the carried Cholesky factor: (status, beta, alpha, W, L)."""
+        torch = _torch()
+        s = self.s
+        M, Cm, Lprev = (self._dev(t, torch.float64, nm, s * s) for t, nm in ((M, "M"), (Cm, "C"), (Lprev, "Lprev")))
+        m = self._dev(m, torch.float64, "m", s)
+        beta = torch.zeros((s, s), dtype=torch.float64, device=M.device)
+        alpha = torch.zeros(s, dtype=torch.float64, device=M.device)
+        W, L = torch.zeros_like(beta), torch.zeros_like(beta)
+        st = torch.zeros(1, dtype=torch.int32, device=M.device)
+        self._check(self._lib.sstep_cg_test_small_solve_carried(self._h, self._ptr(M), self._ptr(Cm), self._ptr(m), self._ptr(Lprev),
+                                                                self._ptr(beta), self._ptr(alpha), self._ptr(W), self._ptr(L),
+                                                                self._ptr(st)), "sstep_cg_test_small_solve_carried")
+        return int(st.item()), beta, alpha, W, L
 
     def test_read_state(self, name: str):
         """One internal array of the current solve state (see sstep_cg.h): blocks come back as (s, n) tensors."""

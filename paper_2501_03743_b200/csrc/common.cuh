@@ -22,6 +22,7 @@ struct ScgState {
     double M[SCG_SMAX * SCG_SMAX];
     double C[SCG_SMAX * SCG_SMAX];
     double m[SCG_SMAX];
+    double Lw[SCG_SMAX * SCG_SMAX];     // Cholesky factor of W (lower triangle, row-major): the next iteration's beta solve reuses it
     // ---- moment form (option "form" = 1): mu^0 = R_1^T r from the update / init kernel, the 2s moments of the last MPK
     double mu0;
     double vm[2 * SCG_SMAX];
@@ -69,6 +70,48 @@ __device__ __forceinline__ double warp_sum_array(const double* p, int cnt, int l
     return v;
 }
 
+// The same sums for K arrays p, p + stride, ... at once (entries beyond kvalid give 0): per array the order of
+// warp_sum_array, bit for bit, but the loads of all K arrays of a pass are in flight together, so a warp that owns several
+// entries of a cross-block finish pays the L2 round trips once instead of K times.
+template <int K>
+__device__ __forceinline__ void warp_sum_arrays(const double* p, int64_t stride, int kvalid, int cnt, int lane, double (&out)[K]) {
+    double a[K][8];
+#pragma unroll
+    for (int q = 0; q < K; q++)
+#pragma unroll
+        for (int k = 0; k < 8; k++) a[q][k] = 0.0;
+    int b = lane;
+    for (; b + 224 < cnt; b += 256) {
+        double v[K][8];
+#pragma unroll
+        for (int q = 0; q < K; q++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) v[q][k] = (q < kvalid) ? __ldcg(p + q * stride + b + 32 * k) : 0.0;
+#pragma unroll
+        for (int q = 0; q < K; q++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) a[q][k] += v[q][k];
+    }
+    {
+        double v[K][8];
+#pragma unroll
+        for (int q = 0; q < K; q++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) v[q][k] = (q < kvalid && b + 32 * k < cnt) ? __ldcg(p + q * stride + b + 32 * k) : 0.0;
+#pragma unroll
+        for (int q = 0; q < K; q++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) a[q][k] += v[q][k];
+    }
+#pragma unroll
+    for (int q = 0; q < K; q++) {
+        double v = ((a[q][0] + a[q][1]) + (a[q][2] + a[q][3])) + ((a[q][4] + a[q][5]) + (a[q][6] + a[q][7]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        out[q] = v;
+    }
+}
+
 template <int L>
 __device__ __forceinline__ double group_sum(double v) {
 #pragma unroll
@@ -110,6 +153,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "DONE_%=:\n\t}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+// one non-blocking probe of the phase with the given parity
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
 }
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
     uint64_t pol;

@@ -72,18 +72,29 @@ __device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * 
     if (!is_last) return;
     __threadfence();
     __shared__ double sW[S * S], sbeta[S * S], salpha[S];
-    for (int e = warp; e < NE; e += nwarps) {
-        const double v = warp_sum_array(partials + (int64_t)e * gridDim.x, (int)gridDim.x, lane);
-        if (lane == 0) fin[e] = v;
+    // a warp owns the entries warp, warp + nwarps, ...; up to three of them per pass, their loads in flight together
+    // (KB = 1, 2 for s = 1, 2: no more registers than the streaming loop of those kernels needs)
+    constexpr int KB = (NE <= 8) ? 1 : (NE <= 16) ? 2 : 3;
+    for (int e = warp; e < NE; e += KB * nwarps) {
+        double v[KB];
+        const int kv = (NE - e + nwarps - 1) / nwarps;
+        warp_sum_arrays<KB>(partials + (int64_t)e * gridDim.x, (int64_t)nwarps * gridDim.x, kv < KB ? kv : KB, (int)gridDim.x, lane, v);
+        if (lane == 0) {
+#pragma unroll
+            for (int q = 0; q < KB; q++)
+                if (e + q * nwarps < NE) fin[e + q * nwarps] = v[q];
+        }
     }
     if (warp == nwarps - 1)
-        for (int e = lane; e < S * S; e += 32) sW[e] = st->W[e];  // W of the previous outer iteration
+        for (int e = lane; e < S * S; e += 32) ssm.L[e] = st->Lw[e];  // Cholesky factor of the previous outer iteration's W
     __syncthreads();
     if (warp == 0) {
         for (int e = lane; e < S * S; e += 32) { st->M[e] = fin[e]; st->C[e] = fin[S * S + e]; }
         if (lane < S) st->m[lane] = fin[2 * S * S + lane];
         if (do_solve) {  // all operands in shared memory: the solves are one long dependent chain
-            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, sW, sbeta, salpha, sW, ssm, lane);
+            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, nullptr, sbeta, salpha, sW, ssm, lane, /*have_L=*/true);
+            if (rc == 0)
+                for (int e = lane; e < S * S; e += 32) st->Lw[e] = ssm.L[e];
             for (int e = lane; e < S * S; e += 32) { st->W[e] = sW[e]; st->beta[e] = sbeta[e]; }
             if (lane < S) st->alpha[lane] = salpha[lane];
             if (lane == 0 && rc != 0) st->status = rc;
@@ -93,7 +104,7 @@ __device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * 
 }
 
 template <int S>
-__global__ void __launch_bounds__(GramCfg<S>::NW * 32, 2)
+__global__ void __launch_bounds__(GramCfg<S>::NW * 32, (S == 1) ? 4 : 2)
 gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ AR, const double* __restrict__ AP,
             const double* __restrict__ r, double* __restrict__ partials, ScgState* __restrict__ st, int do_solve) {
     using Cfg = GramCfg<S>;
@@ -154,10 +165,18 @@ gram_kernel(int64_t n, const double* __restrict__ R, const double* __restrict__ 
     gram_cross_block_finish<S, G, NSL, RG>(red, partials, st, do_solve);
 }
 
-// stand-alone a3 for the test hook: same device function, operands in global memory
-__global__ void small_solve_kernel(int s, const double* M, const double* C, const double* m, const double* Wprev, double* beta,
-                                   double* alpha, double* W, int* status_out) {
+// stand-alone a3 for the test hooks: same device function, operands in global memory.  Lprev != NULL: the carried-factor
+// path of the solver loop (Lprev = Cholesky factor of the previous W; Wprev is then not read); Lout (may be NULL)
+// receives the factor of the new W.
+__global__ void small_solve_kernel(int s, const double* M, const double* C, const double* m, const double* Wprev,
+                                   const double* Lprev, double* beta, double* alpha, double* W, double* Lout, int* status_out) {
     __shared__ SmallSolveSmem ssm;
-    const int rc = warp_small_solve(s, M, C, m, Wprev, beta, alpha, W, ssm, threadIdx.x);
+    if (Lprev) {
+        for (int e = threadIdx.x; e < s * s; e += 32) ssm.L[e] = Lprev[e];
+        __syncwarp();
+    }
+    const int rc = warp_small_solve(s, M, C, m, Wprev, beta, alpha, W, ssm, threadIdx.x, Lprev != nullptr);
+    if (Lout && rc == 0)
+        for (int e = threadIdx.x; e < s * s; e += 32) Lout[e] = ssm.L[e];
     if (threadIdx.x == 0) status_out[0] = rc;
 }

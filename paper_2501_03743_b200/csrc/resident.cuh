@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
             sAP[j * RPB + lr] = p.AP[(size_t)row * S + j];
         }
     }
-    for (int e = tid; e < S * S; e += bd) { sW[e] = st->W[e]; sbeta[e] = st->beta[e]; }
+    for (int e = tid; e < S * S; e += bd) { sW[e] = st->W[e]; sbeta[e] = st->beta[e]; ssm.L[e] = st->Lw[e]; }
     if (tid < S) salpha[tid] = st->alpha[tid];
     int k_outer = st->k;
     const double rho0 = st->rho0, rtol = st->rtol;
@@ -226,7 +226,8 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
         }
         __syncthreads();
         if (warp == 0) {
-            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, sW, sbeta, salpha, sW, ssm, lane);
+            // (ssm.L carries the Cholesky factor of W from one outer iteration to the next: one factorisation each)
+            const int rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, nullptr, sbeta, salpha, sW, ssm, lane, /*have_L=*/true);
             if (lane == 0) s_rc = rc;
         }
         __syncthreads();
@@ -310,6 +311,7 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
         __syncthreads();
         for (int e = tid; e < S * S; e += bd) {
             st->W[e] = sW[e];
+            if (status != 2) st->Lw[e] = ssm.L[e];
             st->beta[e] = sbeta[e];
             st->M[e] = fin[e];
             st->C[e] = fin[S * S + e];

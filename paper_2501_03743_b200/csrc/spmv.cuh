@@ -157,9 +157,12 @@ __global__ void __launch_bounds__(WPC * 32, MINB) spmv_bulk_kernel(int n, int nn
         const int b_end = __shfl_sync(0xffffffffu, bulk_end, 0);
         const int b_a0 = __shfl_sync(0xffffffffu, a0, 0);
         const int b_nz1 = __shfl_sync(0xffffffffu, nz1, 0);
-        for (int e = b_end + lane; e < b_nz1; e += 32) {
-            dv[e - b_a0] = va[e];
-            dc[e - b_a0] = ci[e];
+        if (b_end < b_nz1) {  // (warp-uniform; only the last tile of a matrix with nnz % 4 != 0 comes here)
+            for (int e = b_end + lane; e < b_nz1; e += 32) {
+                dv[e - b_a0] = va[e];
+                dc[e - b_a0] = ci[e];
+            }
+            __syncwarp();  // other lanes read these entries in load_frag behind a per-lane mbarrier wait only
         }
     };
     auto tile_bounds = [&](int i, int& nz0, int& nz1) {  // lane 0 only

@@ -1,0 +1,188 @@
+// spmv_cta.cuh -- step a1, thread-per-row matrices (mean row <= 8 entries: every 7-point config): the Jacobi-fused CSR
+// SpMV of the matrix-powers kernel (Alg. 4) with a CTA-wide producer / consumer TMA pipeline.
+//
+// Why a second bulk-staged kernel (round 2).  The per-warp rings of spmv_bulk_kernel keep 24 warps x 2 slots x 2 arrays
+// = 96 bulk copies of ~1.3 KB in flight per SM.  Measured on this B200 with a pure streaming kernel (_work probe,
+// numbers in DESIGN.md section 6): the 1-D bulk-copy path of an SM runs at full speed only up to ~32 copies in flight --
+// 16-32 copies of >= 4 KB stream 7.2-7.3 TB/s from HBM and 18 TB/s from L2, 48 copies 6.0-7.5 TB/s from either, 96
+// copies 3.6 TB/s.  So the bytes in flight must come from FEW, LARGE copies: here one producer warp per CTA streams
+// tiles of TR = 256 rows (colidx + vals of the whole tile = two copies of ~14 KB + ~7 KB) into a ring of D stages, and
+// TR/32 consumer warps compute from shared memory: 3 CTAs x D = 3 stages x 2 = 18 copies and ~190 KB in flight per SM.
+//
+//   producer (warp TR/32):  wait empty[st] -> rowptr of the tile's ends -> expect_tx(full[st]) + 2 bulk copies
+//   consumer warp w:        rows tile*TR + 32 w + lane; (rowptr pair fetched one tile ahead) wait full[st] -> fragment
+//                           (<= 8 entries) to registers -> x gathers issued -> arrive empty[st] -> FMAs, epilogue, stores
+// Arithmetic per row, epilogue modes, 1/a_ii from the row's own diagonal entry and the moment partials (MOM) are those
+// of spmv_bulk_kernel at L = 1 (spmv.cuh), bit for bit.  Tiles are dealt to CTAs round-robin, so the grid sweeps one
+// contiguous window of rows (gather locality in L1 / L2).
+#pragma once
+#include "common.cuh"
+#include "spmv.cuh"
+
+template <int D, int TR, int CAPT>
+struct SpmvCtaCfg {
+    static constexpr int NCW = TR / 32;                 // consumer warps
+    static constexpr int THREADS = TR + 32;             // + one producer warp
+    static constexpr size_t STAGE = (size_t)CAPT * 12;  // vals then cols of one stage
+    static constexpr size_t SMEM = (size_t)D * STAGE + (size_t)D * 16 /* full, empty */ + (size_t)D * 8 /* a0 per stage */;
+    static_assert(CAPT % 4 == 0 && TR % 32 == 0, "stage sub-buffers must stay 16-byte aligned");
+};
+
+template <int D, int TR, int CAPT, bool MOM, int MINB>
+__global__ void __launch_bounds__(TR + 32, MINB)
+spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restrict__ ci, const double* __restrict__ va,
+                const double* __restrict__ x, double* __restrict__ y, double* __restrict__ yjac,
+                const double* __restrict__ xprev, int mode, const ScgState* __restrict__ st, int num_tiles,
+                double* __restrict__ mom_a, double* __restrict__ mom_b) {
+    using Cfg = SpmvCtaCfg<D, TR, CAPT>;
+    constexpr int NCW = Cfg::NCW, U = 8;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* svals = reinterpret_cast<double*>(smem_raw);                                  // [D][CAPT]
+    int* scols = reinterpret_cast<int*>(smem_raw + (size_t)D * CAPT * sizeof(double));    // [D][CAPT]
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * Cfg::STAGE);
+    uint64_t* empty = full + D;
+    int* s_a0 = reinterpret_cast<int*>(empty + D);                                        // [D] first staged nnz index
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int d = 0; d < D; d++) { mbar_init(&full[d], 1); mbar_init(&empty[d], NCW); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int my_tiles = ((int)blockIdx.x < num_tiles) ? (num_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    auto tile_row0 = [&](int i) { return ((int)blockIdx.x + i * (int)gridDim.x) * TR; };
+
+    if (warp == NCW) {
+        // ------------------------------------------------------------------ producer warp
+        // rowptr / colidx / vals are written by no kernel: the first D tiles are staged ahead of the dependency wait (with
+        // a programmatic dependent launch they stream while the predecessor drains); if the solver has stopped, producer
+        // and consumers agree to handle exactly those D tiles (the consumers only hand them back)
+        const uint64_t policy = l2_policy_evict_first();
+        int tiles_eff = my_tiles;
+        for (int i = 0; i < tiles_eff; i++) {
+            const int sl = i % D;
+            if (i == D) {  // ring filled once: from here on the solver's state decides (a stopped solver streams no further)
+                pdl_wait();
+                if (st && st->status != SCG_RUNNING) break;
+            }
+            if (i >= D) mbar_wait(&empty[sl], (uint32_t)(((i / D) - 1) & 1));
+            const int row0 = tile_row0(i);
+            int row1 = row0 + TR;
+            if (row1 > n) row1 = n;
+            int nz0 = 0, nz1 = 0;
+            if (lane == 0) { nz0 = rp[row0]; nz1 = rp[row1]; }
+            nz0 = __shfl_sync(0xffffffffu, nz0, 0);
+            nz1 = __shfl_sync(0xffffffffu, nz1, 0);
+            const int a0 = nz0 & ~3;
+            int bulk_end = (nz1 + 3) & ~3;
+            const int lim = nnz & ~3;
+            if (bulk_end > lim) bulk_end = lim;
+            if (bulk_end < a0) bulk_end = a0;
+            const int cnt = bulk_end - a0;
+            double* dv = svals + (size_t)sl * CAPT;
+            int* dc = scols + (size_t)sl * CAPT;
+            // ragged tail of the arrays (at most 3 entries of the whole matrix) by plain loads
+            for (int e = bulk_end + lane; e < nz1; e += 32) { dv[e - a0] = va[e]; dc[e - a0] = ci[e]; }
+            if (lane == 0) s_a0[sl] = a0;
+            __syncwarp();  // the stores above are ordered before lane 0's releasing arrive
+            if (lane == 0) {
+                fence_proxy_async_smem();
+                if (cnt > 0) {
+                    mbar_expect_tx(&full[sl], (uint32_t)cnt * 12u);
+                    bulk_g2s(dv, va + a0, (uint32_t)cnt * 8u, &full[sl], policy);
+                    bulk_g2s(dc, ci + a0, (uint32_t)cnt * 4u, &full[sl], policy);
+                } else {
+                    mbar_arrive(&full[sl]);
+                }
+            }
+        }
+        if (MOM) spmv_moment_finish(0.0, 0.0, mom_a, mom_b);  // (block-wide reduction: every warp takes part)
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumer warps
+    double ma = 0.0, mb = 0.0;
+    const bool jac = yjac != nullptr;
+    int lo_n = 0, hi_n = 0;
+    auto row_bounds = [&](int i, int& lo, int& hi) {
+        lo = hi = 0;
+        if (i < my_tiles) {
+            const int row = tile_row0(i) + warp * 32 + lane;
+            if (row < n) { lo = rp[row]; hi = rp[row + 1]; }
+        }
+    };
+    row_bounds(0, lo_n, hi_n);  // (rowptr only: may run ahead of the dependency wait)
+    pdl_wait();
+    pdl_launch();
+    const bool running = !(st && st->status != SCG_RUNNING);
+    const int tiles_eff = running ? my_tiles : (my_tiles < D ? my_tiles : D);  // stopped: only what the prologue staged
+    for (int i = 0; i < tiles_eff; i++) {
+        const int sl = i % D;
+        const int lo = lo_n, hi = hi_n;
+        const int row = tile_row0(i) + warp * 32 + lane;
+        row_bounds(i + 1, lo_n, hi_n);
+        mbar_wait(&full[sl], (uint32_t)((i / D) & 1));
+        if (!running) {  // stopped solver: hand the stage back, compute nothing
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[sl]);
+            continue;
+        }
+        const int a0 = s_a0[sl];
+        const double* sv = svals + (size_t)sl * CAPT - a0;
+        const int* sc = scols + (size_t)sl * CAPT - a0;
+        int c[U];
+        double v[U], xv[U];
+        double diag = 0.0;
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int kk = lo + u;
+            const bool ok = kk < hi;
+            c[u] = ok ? sc[kk] : -1;
+            v[u] = ok ? sv[kk] : 0.0;
+            if (c[u] == row) diag = v[u];
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
+        double xrow = 0.0, xpv = 0.0;
+        if ((MOM || (jac && mode != 0)) && row < n) {
+            xrow = x[row];
+            if (mode == 2) xpv = xprev[row];
+        }
+        double rem = 0.0;
+        for (int k0 = lo + U; k0 < hi; k0 += U) {  // rows longer than U entries: further batches
+            int cc[U];
+            double vv[U], xx[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int kk = k0 + u;
+                const bool ok = kk < hi;
+                cc[u] = ok ? sc[kk] : -1;
+                vv[u] = ok ? sv[kk] : 0.0;
+                if (cc[u] == row) diag = vv[u];
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) xx[u] = (cc[u] >= 0) ? x[cc[u]] : 0.0;
+#pragma unroll
+            for (int u = 0; u < U; u++) rem = fma(vv[u], xx[u], rem);
+        }
+        __syncwarp();  // every lane has read the stage
+        if (lane == 0) mbar_arrive(&empty[sl]);
+        double acc = 0.0;
+#pragma unroll
+        for (int u = 0; u < U; u++) acc = fma(v[u], xv[u], acc);
+        acc += rem;
+        if (row < n) {
+            y[row] = acc;
+            if (MOM) ma = fma(xrow, acc, ma);
+            if (jac) {
+                double z = __drcp_rn(diag) * acc;
+                if (MOM) mb = fma(z, acc, mb);
+                if (mode == 1) z = z - xrow;
+                else if (mode == 2) z = 2.0 * (z - xrow) - xpv;
+                yjac[row] = z;
+            }
+        }
+    }
+    if (MOM) spmv_moment_finish(ma, mb, mom_a, mom_b);
+}

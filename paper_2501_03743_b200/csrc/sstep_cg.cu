@@ -10,12 +10,14 @@
 #include "common.cuh"
 #include "gram.cuh"
 #include "gram_tma.cuh"
+#include "measure.cuh"
 #include "moment.cuh"
 #include "mpk_wave.cuh"
 #include "pcg.cuh"
 #include "reorder.cuh"
 #include "resident.cuh"
 #include "spmv.cuh"
+#include "spmv_cta.cuh"
 #include "update.cuh"
 #include "update_tma.cuh"
 
@@ -38,6 +40,13 @@ constexpr int BULK_CAP2 = 448, BULK_WPC2 = 10;    // tiles up to 445 entries (16
 constexpr int BULK_CAP2B = 512, BULK_WPC2B = 8;   // tiles up to 509 entries (16 rows x 31)
 constexpr int BULK_CAP1 = 1024, BULK_WPC1 = 4;    // L = 1, depth 2
 constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D * cap * 12 + (size_t)wpc * D * 8; }
+// CTA-pipelined SpMV (spmv_cta.cuh), thread-per-row matrices: tiles of 256 rows, stage capacity 1800 entries (a 7-point
+// tile holds <= 1792; three stages x three CTAs = 194 KB of shared memory per SM, ~33 KB left for L1)
+constexpr int CTA_TR = 256, CTA_CAPT = 1800;
+// wavefront matrix-powers kernel (mpk_wave.cuh): ring stages, stages per work item (item = MW_SPI * CTA_TR rows), most levels per pass
+constexpr int MW_D = 2, MW_SPI = 2, MW_MAXLEV = 5;
+constexpr int MW_SMALL_TR = 64, MW_SMALL_CAPT = 520;  // option mpk_block_rows = 64: items of 64 rows (rows of <= 8 entries)
+constexpr bool MW_AUTO = false;  // (selected automatically only once it beats the separate SpMVs)
 
 }  // namespace
 
@@ -70,9 +79,12 @@ struct sstep_cg {
     int lanes = 1;
     bool bulk = false;
     int bulk_cap = 256, bulk_wpc = 8;
+    bool cta = false;             // thread-per-row matrices: CTA-pipelined SpMV (spmv_cta.cuh) instead of the per-warp rings
+    int cta_depth = 3, cta_minb = 3, cta_tiles = 0;
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0, pcg_grid = 0;
     bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
+    int gram_tile = 0, gram_depth = 0, update_tile = 0, update_depth = 0;  // staged kernels: rows per tile, ring slots (0 = not staged)
     int64_t num_tiles = 0;
     int max_row_len = 0;
     double dinv_uniform = 0.0;  // 1 / a_ii if the diagonal is constant (then the update kernels skip the dinv stream), else 0
@@ -84,7 +96,8 @@ struct sstep_cg {
     int cm_levels = 0, cm_comps = 0, far_permille = 0;
     // wavefront-fused matrix-powers kernel (mpk_wave.cuh): the CSR arrays are read from HBM once per pass of `mw_levels` levels
     bool mpk_fused = false;
-    int bandwidth = 0, mw_tpb = 0, mw_nb = 0, mw_lag = 0, mw_lag_dep = 0, mw_levels = 0;
+    int bandwidth = 0, mw_block = 0, mw_nb = 0, mw_lag = 0, mw_lag_dep = 0, mw_levels = 0, mw_grid = 0;
+    size_t mw_sync_ints = 0;
     int* mw_sync = nullptr;  // [s * nb] done counters, then [s] watermarks
     // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
     bool resident = false;
@@ -159,9 +172,33 @@ bulk_fn_t bulk_kernel_for(int depth, bool mom, int cap) {
     return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth);
 }
 
+template <bool MOM>
+bulk_fn_t cta_kernel_mom(int depth, int minb) {
+    if (minb == 2) {
+        switch (depth) {
+            case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 2>;
+            case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 2>;
+            default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 2>;
+        }
+    }
+    switch (depth) {
+        case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 3>;
+        case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 3>;
+        default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 3>;
+    }
+}
+bulk_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
+    return mom ? cta_kernel_mom<true>(h->cta_depth, h->cta_minb) : cta_kernel_mom<false>(h->cta_depth, h->cta_minb);
+}
+size_t cta_smem_for(int depth) { return (size_t)depth * CTA_CAPT * 12 + (size_t)depth * 24; }
+
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
+    if (L == 1 && h->cta) {
+        return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, CTA_TR + 32, cta_smem_for(h->cta_depth), sm, (int)h->n,
+                        (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->cta_tiles, mom_a, mom_b);
+    }
     if (h->bulk) {
         return launch_k(h, bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr, h->bulk_cap), h->spmv_grid, h->bulk_wpc * 32,
                         bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc), sm, (int)h->n, (int)h->nnz, h->rp, h->ci, h->va,
@@ -188,6 +225,21 @@ template <int L>
 cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
+    if (L == 1 && h->cta) {
+        const size_t smem = cta_smem_for(h->cta_depth);
+        for (int mom = 0; mom < 2; mom++) {
+            e = cudaFuncSetAttribute(cta_kernel_for(h, mom != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cta_kernel_for(h, h->form != 0 || h->method == 1), CTA_TR + 32, smem);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        if (occ > h->cta_minb) occ = h->cta_minb;
+        const int64_t cap = (int64_t)occ * h->num_sms;
+        h->spmv_grid = (int)(h->cta_tiles < cap ? h->cta_tiles : cap);
+        if (h->spmv_grid < 1) h->spmv_grid = 1;
+        return cudaSuccess;
+    }
     if (h->bulk) {
         auto k = bulk_kernel_for<L>(h->spmv_depth, h->form != 0 || h->method == 1, h->bulk_cap);
         const size_t smem = bulk_smem_for(h->spmv_depth, h->bulk_cap, h->bulk_wpc);
@@ -253,6 +305,8 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
             h->gram_grid = (int)(want < cap ? want : cap);
             if (h->gram_grid < h->gram_grid_reg) h->gram_grid_reg = h->gram_grid;  // partials are sized by gram_grid
         }
+        h->gram_tile = h->staged ? TC::T : 0;
+        h->gram_depth = h->staged ? TC::D : 0;
         return cudaSuccess;
     }
     if (h->staged && aligned16(R) && aligned16(AR) && aligned16(AP) && aligned16(r)) {
@@ -285,6 +339,8 @@ cudaError_t update_SM(sstep_cg* h, cudaStream_t sm, bool configure, double* R, c
             h->update_grid = (int)(want < cap ? want : cap);
             if (h->update_grid < h->update_grid_reg) h->update_grid_reg = h->update_grid;
         }
+        h->update_tile = h->staged ? TC::T : 0;
+        h->update_depth = h->staged ? TC::D : 0;
         return cudaSuccess;
     }
     if (h->staged && aligned16(R) && aligned16(AR) && aligned16(P) && aligned16(AP) && aligned16(x) && aligned16(r)) {
@@ -360,18 +416,21 @@ cudaError_t resident_op(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ
 cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, const ScgState* st) {
     const int64_t n = h->n;
     if (h->mpk_fused) {  // wavefront order: one launch per pass of mw_levels levels (mpk_wave.cuh)
-        cudaError_t e = cudaMemsetAsync(h->mw_sync, 0, sizeof(int) * ((size_t)h->s * h->mw_nb + 32 * (size_t)h->s + 32), sm);
-        if (e != cudaSuccess) return e;
         for (int j0 = 0; j0 < h->s; j0 += h->mw_levels) {
+            cudaError_t e = cudaMemsetAsync(h->mw_sync, 0, sizeof(int) * h->mw_sync_ints, sm);
+            if (e != cudaSuccess) return e;
             MpkWaveParams p;
             p.n = (int)n; p.nnz = (int)h->nnz; p.s = h->s;
             p.j0 = j0; p.nlev = (h->s - j0 < h->mw_levels) ? h->s - j0 : h->mw_levels;
-            p.tpb = h->mw_tpb; p.nb = h->mw_nb; p.lag = h->mw_lag; p.lag_dep = h->mw_lag_dep; p.basis = h->basis;
+            p.nb = h->mw_nb; p.lag = h->mw_lag; p.dep = h->mw_lag_dep; p.bp = h->mw_lag - h->mw_lag_dep; p.basis = h->basis;
             p.rp = h->rp; p.ci = h->ci; p.va = h->va; p.R = R; p.AR = AR; p.st = st;
-            p.done = h->mw_sync; p.watermark = h->mw_sync + ((size_t)h->s * h->mw_nb + 31) / 32 * 32;
-            void* args[] = {&p};
-            e = cudaLaunchCooperativeKernel((const void*)mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, dim3(h->spmv_grid), dim3(BULK_WPC * 32), args,
-                                            bulk_smem_for(2, BULK_CAP, BULK_WPC), sm);
+            p.watermark = h->mw_sync; p.done = h->mw_sync + 32 * MW_MAXLEV;
+            if (h->mw_block == MW_SMALL_TR)  // (64-row items: dependency stress on small matrices, tests only)
+                e = launch_k(h, mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, h->mw_grid, MW_SMALL_TR + 32,
+                             MpkWaveCfg<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>::SMEM, sm, p);
+            else
+                e = launch_k(h, mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, h->mw_grid, CTA_TR + 32,
+                             MpkWaveCfg<MW_D, CTA_TR, CTA_CAPT, MW_SPI>::SMEM, sm, p);
             if (e != cudaSuccess) return e;
             h->launches++;
         }
@@ -503,7 +562,7 @@ int setup_analyze(sstep_cg* h) {
     CK(cudaStreamSynchronize(sm));
     if (hs[0]) {
         char buf[160];
-        snprintf(buf, sizeof buf, "setup: invalid matrix (flags %d: 1 rowptr, 2 column index, 4 diagonal missing or <= 0)", hs[0]);
+        snprintf(buf, sizeof buf, "setup: invalid matrix (flags %d: 1 rowptr, 2 column index, 4 diagonal missing, duplicated or <= 0)", hs[0]);
         free_problem(h);
         return fail(h, SSTEP_CG_ERR_MATRIX, buf);
     }
@@ -637,6 +696,27 @@ int setup_spmv_variant(sstep_cg* h) {
         free_problem(h);
         return fail(h, SSTEP_CG_ERR_ARG, "setup: bulk SpMV forced but a tile exceeds the staging capacity or arrays are not 16 B aligned");
     }
+    // thread-per-row matrices whose 256-row tiles fit a stage: the CTA-pipelined kernel (few large bulk copies in flight,
+    // spmv_cta.cuh) replaces the per-warp rings -- auto, or forced with spmv_variant = 3 (2 keeps the per-warp rings)
+    h->cta = false;
+    if (((h->spmv_variant == 0 && h->bulk && h->bulk_cap == BULK_CAP) || h->spmv_variant == 3) && L == 1 && aligned &&
+        n + 2 * CTA_TR < (int64_t(1) << 31)) {
+        const int64_t tiles = (n + CTA_TR - 1) / CTA_TR;
+        CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
+        tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, CTA_TR, tiles, h->iscratch + 2);
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
+        CK(cudaStreamSynchronize(sm));
+        if (hs[2] + 3 <= CTA_CAPT) {
+            h->cta = true;
+            h->cta_tiles = (int)tiles;
+        }
+    }
+    if (h->spmv_variant == 3 && !h->cta) {
+        free_problem(h);
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: CTA-pipelined SpMV forced but it needs one lane per row, 16 B aligned arrays and "
+                                         "256-row tiles of at most 1797 entries");
+    }
     h->lanes = L;
     return 0;
 }
@@ -661,79 +741,75 @@ int setup_block_kernels(sstep_cg* h) {
     return 0;
 }
 
-// shape of the experimental wavefront-fused matrix-powers kernel
+// shape of the wavefront-ordered matrix-powers kernel (mpk_wave.cuh)
 int setup_mpk_wave(sstep_cg* h) {
     const int64_t n = h->n;
     const int64_t nnz = h->nnz;
     const int s = h->s;
     cudaStream_t sm = h->stream;
-    const int* rowptr = h->rp;
-    const int* colidx = h->ci;
     int hs[4] = {0, 0, 0, 0};
-    // banded matrices on the thread-per-row bulk SpMV shape, s >= 2: blocks of 8192 rows, dependency distance
-    // ceil(bw / B) + 1 blocks plus a slack, as many levels per pass as keep the re-read window under 48 MB of L2
     h->mpk_fused = false;
     h->mw_levels = 0;
-    // (not chosen automatically: see the measurements in mpk_wave.cuh -- it halves the DRAM traffic of the MPK but is
-    // still slower than the separate SpMVs)
-    if (h->mpk_fused_opt == 2 && h->bulk && h->lanes == 1 && h->bulk_cap == BULK_CAP && h->spmv_depth == 2 && h->form == 0 &&
-        h->method == 0 && s >= 2 && n % 4 == 0) {
-        int coop = 0;
-        CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device));
+    // thread-per-row matrices on the CTA-pipelined SpMV shape, Gram form, s >= 2, n % 4 == 0 (32-byte aligned columns of
+    // R), 16-byte aligned rowptr, and a bandwidth whose re-read window fits the fast part of L2.  Auto: only when the
+    // matrix is much larger than L2 (otherwise the separate SpMVs already re-read it from L2)
+    const bool applicable = h->cta && h->form == 0 && h->method == 0 && s >= 2 && n % 4 == 0 && (((uintptr_t)h->rp) & 15) == 0;
+    const bool wanted = h->mpk_fused_opt == 2 || (MW_AUTO && h->mpk_fused_opt == 0 && 12.0 * (double)nnz > 400.0e6);
+    if (applicable && wanted) {
         CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
-        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, rowptr, colidx, h->iscratch + 3);
+        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, h->rp, h->ci, h->iscratch + 3);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
         CK(cudaStreamSynchronize(sm));
         h->bandwidth = hs[3];
-        // shape: small blocks (fine-grained signalling), g levels per pass, slack = 4 x the tiles the grid holds in flight
-        const int64_t gwarps = (int64_t)h->spmv_grid * BULK_WPC;
-        int64_t B = 8192;  // 256 tiles: a power of two (cheap tile decoding in the kernel)
-        if (h->mpk_block_opt) B = h->mpk_block_opt;
-        if ((B / 32) & (B / 32 - 1)) B = 0;  // not 32 * 2^k: not applicable
-        const int64_t nb = B ? (n + B - 1) / B : 0;
-        const int64_t lag_dep = B ? (h->bandwidth + B - 1) / B + 1 : 0;
-        if (!B) { coop = 0; B = 32; }
-        const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 16.0;
-        int g = s < 5 ? s : 5;  // (the kernel keeps the watermarks of up to 4 predecessor levels in registers)
-        int64_t slack = 0, lag = 0;
-        for (;; g--) {  // largest g whose re-read window (g - 1)(bw + B + slack rows) fits 48 MB of L2
-            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
-            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
-            lag = lag_dep + slack;
-            if (g <= 1 || (double)(g - 1) * (double)(lag * B) * row_bytes <= 48.0e6) break;
+        using WC = MpkWaveCfg<MW_D, CTA_TR, CTA_CAPT, MW_SPI>;
+        using WS = MpkWaveCfg<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>;
+        const bool small = h->mpk_block_opt == MW_SMALL_TR && h->max_row_len <= 8;
+        int occ = 0;
+        if (small) {
+            CK(cudaFuncSetAttribute(mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WS::SMEM));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, WS::THREADS, WS::SMEM));
+        } else {
+            CK(cudaFuncSetAttribute(mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WC::SMEM));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, WC::THREADS, WC::SMEM));
         }
-        if (h->mpk_levels_opt) {
-            g = h->mpk_levels_opt < s ? h->mpk_levels_opt : s;
-            if (g > 5) g = 5;
-            slack = (4 * gwarps * 32 / (g > 1 ? g : 1) + B - 1) / B;
-            if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
-            lag = lag_dep + slack;
-        }
-        if (coop && g >= 2 && (nb >= 4 * lag || h->mpk_fused_opt == 2)) {
-            const int passes = (s + g - 1) / g;
-            h->mw_levels = (s + passes - 1) / passes;
-            h->mw_tpb = (int)(B / 32);
-            h->mw_nb = (int)nb;
-            h->mw_lag = (int)lag;
-            h->mw_lag_dep = (int)lag_dep;
-            cudaError_t e = cudaFuncSetAttribute(mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 (int)bulk_smem_for(2, BULK_CAP, BULK_WPC));
-            int occ = 0;
-            if (e == cudaSuccess)
-                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<2, BULK_CAP, BULK_WPC>, BULK_WPC * 32,
-                                                                  bulk_smem_for(2, BULK_CAP, BULK_WPC));
-            CK(e);
-            if ((int64_t)occ * h->num_sms >= h->spmv_grid) {
-                CK(cudaMalloc(&h->mw_sync, sizeof(int) * ((size_t)s * nb + 32 * (size_t)s + 32)));
+        if (occ > 3) occ = 3;
+        if (occ >= 1) {
+            const int64_t B = small ? WS::BR : WC::BR;
+            const int64_t nb = (n + B - 1) / B;
+            const int64_t grid = (int64_t)occ * h->num_sms < nb ? (int64_t)occ * h->num_sms : nb;
+            const int64_t dep = (h->bandwidth + B - 1) / B + 1;
+            const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 24.0;
+            // levels per pass: the largest g whose re-read window (g - 1) * lag blocks stays within ~56 MB of L2; the slack
+            // covers the items the grid has in flight (about one per CTA and level)
+            int g = s < MW_MAXLEV ? s : MW_MAXLEV;
+            if (h->mpk_levels_opt) g = h->mpk_levels_opt < g ? h->mpk_levels_opt : g;
+            int64_t slack = 0, lag = 0;
+            for (;; g--) {
+                slack = (2 * grid) / (g > 1 ? g : 1) + 8;
+                if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
+                lag = dep + slack;
+                if (g <= 2 || h->mpk_levels_opt || ((double)(g - 1) * (double)lag + (double)slack) * (double)B * row_bytes <= 56.0e6) break;
+            }
+            const bool fits = ((double)(g - 1) * (double)lag + (double)slack) * (double)B * row_bytes <= 80.0e6;
+            if (g >= 2 && (fits || h->mpk_fused_opt == 2) && (nb + (int64_t)(g - 1) * lag) * g < (int64_t(1) << 31)) {
+                const int passes = (s + g - 1) / g;
+                h->mw_levels = (s + passes - 1) / passes;
+                h->mw_block = (int)B;
+                h->mw_nb = (int)nb;
+                h->mw_lag = (int)lag;
+                h->mw_lag_dep = (int)dep;
+                h->mw_grid = (int)grid;
+                h->mw_sync_ints = 32 * (size_t)MW_MAXLEV + (size_t)MW_MAXLEV * nb;
+                CK(cudaMalloc(&h->mw_sync, sizeof(int) * h->mw_sync_ints));
                 h->mpk_fused = true;
             }
         }
     }
     if (h->mpk_fused_opt == 2 && !h->mpk_fused) {
         free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: fused matrix-powers kernel forced but not applicable (needs the thread-per-row bulk SpMV, "
-                                         "s >= 2, form = 0, n % 4 == 0 and a bandwidth whose re-read window fits L2)");
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: wavefront matrix-powers kernel forced but not applicable (needs the CTA-pipelined "
+                                         "thread-per-row SpMV, s >= 2, form = 0, n % 4 == 0, 16-byte aligned rowptr)");
     }
     return 0;
 }
@@ -894,7 +970,9 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     if (!h || !key) return SSTEP_CG_ERR_ARG;
     const std::string k(key);
     if (k == "basis" && (value == 0 || value == 1)) h->basis = (int)value;
-    else if (k == "spmv_variant" && value >= 0 && value <= 2) h->spmv_variant = (int)value;
+    else if (k == "spmv_variant" && value >= 0 && value <= 3) h->spmv_variant = (int)value;
+    else if (k == "spmv_cta_depth" && value >= 2 && value <= 4) h->cta_depth = (int)value;
+    else if (k == "spmv_cta_per_sm" && value >= 2 && value <= 3) h->cta_minb = (int)value;
     else if (k == "lanes" && (value == 0 || value == 1 || value == 2 || value == 4 || value == 8 || value == 16 || value == 32))
         h->lanes_opt = (int)value;
     else if (k == "use_graph" && (value == 0 || value == 1)) h->use_graph = (int)value;
@@ -906,8 +984,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
     else if (k == "method" && (value == 0 || value == 1)) h->method = (int)value;
     else if (k == "mpk_fused" && value >= 0 && value <= 2) h->mpk_fused_opt = (int)value;
-    else if (k == "mpk_block_rows" && value >= 0 && value % 32 == 0 && value <= (1 << 30) && ((value / 32) & (value / 32 - 1)) == 0)
-        h->mpk_block_opt = (int)value;  // 32 * 2^k rows
+    else if (k == "mpk_block_rows" && (value == 0 || value == MW_SMALL_TR)) h->mpk_block_opt = (int)value;
     else if (k == "mpk_levels" && value >= 0 && value <= SSTEP_CG_SMAX) h->mpk_levels_opt = (int)value;
     else if (k == "mpk_slack" && value >= -1 && value <= (1 << 20)) h->mpk_slack_opt = (int)value;
     else if (k == "pdl" && (value == 0 || value == 1)) h->pdl = (int)value;
@@ -919,7 +996,8 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     if (!h || !key || !value) return SSTEP_CG_ERR_ARG;
     const std::string k(key);
     if (k == "lanes") *value = h->lanes;
-    else if (k == "spmv_bulk") *value = h->bulk ? 1 : 0;
+    else if (k == "spmv_bulk") *value = (h->bulk || h->cta) ? 1 : 0;
+    else if (k == "spmv_cta") *value = h->cta ? 1 : 0;
     else if (k == "spmv_grid") *value = h->spmv_grid;
     else if (k == "spmv_depth") *value = h->spmv_depth;
     else if (k == "bulk_cap") *value = h->bulk ? h->bulk_cap : 0;
@@ -927,6 +1005,12 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "form") *value = h->form;
     else if (k == "gram_grid") *value = h->gram_grid;
     else if (k == "update_grid") *value = h->update_grid;
+    else if (k == "gram_grid_reg") *value = h->gram_grid_reg;
+    else if (k == "update_grid_reg") *value = h->update_grid_reg;
+    else if (k == "gram_tile_rows") *value = h->gram_tile;
+    else if (k == "gram_ring_depth") *value = h->gram_depth;
+    else if (k == "update_tile_rows") *value = h->update_tile;
+    else if (k == "update_ring_depth") *value = h->update_depth;
     else if (k == "max_row_len") *value = h->max_row_len;
     else if (k == "num_sms") *value = h->num_sms;
     else if (k == "kernels_per_outer") *value = kernels_per_outer(h);
@@ -939,7 +1023,8 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "bandwidth") *value = h->bandwidth;
     else if (k == "uniform_diagonal") *value = h->dinv_uniform > 0.0 ? 1 : 0;
     else if (k == "mpk_levels_per_pass") *value = h->mw_levels;
-    else if (k == "mpk_block_rows") *value = (int64_t)h->mw_tpb * 32;
+    else if (k == "mpk_block_rows") *value = h->mw_block;
+    else if (k == "mpk_grid") *value = h->mw_grid;
     else if (k == "mpk_lag") *value = h->mw_lag;
     else if (k == "mpk_lag_dep") *value = h->mw_lag_dep;
     else if (k == "reordered") *value = h->reordered ? 1 : 0;
@@ -1024,11 +1109,18 @@ int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
     if (!h || k_outer < 0) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "iterate: call solve_begin first");
     if (h->resident) {  // one cooperative launch runs up to k_outer outer iterations (stops on the device at convergence)
-        if (k_outer == 0) return 0;
-        CK(cudaMemsetAsync(&h->st->grid_bar, 0, 33 * sizeof(unsigned int), h->stream));
-        CK(resident_op(h, h->stream, 1, k_outer, nullptr));
-        h->launches++;
-        h->graph_launches++;
+        // the grid barrier counts arrivals in 32 bits (resident.cuh): at most 2^31 arrivals per launch, i.e. kcap outer
+        // iterations of s + 1 barriers each; longer runs are split into several launches (each re-reads the state and
+        // exits at once when the solver has stopped)
+        const int64_t kcap = (int64_t(1) << 31) / ((int64_t)h->res_grid * (h->s + 1)) - 1;
+        for (int64_t done = 0; done < k_outer;) {
+            const int k = (int)((k_outer - done < kcap) ? k_outer - done : kcap);
+            CK(cudaMemsetAsync(&h->st->grid_bar, 0, 33 * sizeof(unsigned int), h->stream));
+            CK(resident_op(h, h->stream, 1, k, nullptr));
+            h->launches++;
+            h->graph_launches++;
+            done += k;
+        }
         return 0;
     }
     for (int i = 0; i < k_outer; i++) {
@@ -1130,6 +1222,23 @@ int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
     return rc;
 }
 
+int sstep_cg_solve_peek(sstep_cg_t* h, sstep_cg_result* out) {
+    if (!h || !out) return SSTEP_CG_ERR_ARG;
+    if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "solve_peek: call solve_begin first");
+    cudaStream_t sm = h->stream;
+    CK(cudaMemcpyAsync(&h->h_hdr[0], h->st, sizeof(Header), cudaMemcpyDeviceToHost, sm));
+    CK(cudaStreamSynchronize(sm));
+    const Header hd = h->h_hdr[0];
+    out->status = hd.status;  // SSTEP_CG_RUNNING while the stop test has not fired
+    out->outer_iters = hd.k;
+    out->cg_equiv_iters = (int64_t)hd.k * h->s;
+    out->r0_norm = sqrt(hd.rho0);
+    out->relres = hd.rho0 > 0.0 ? sqrt(hd.rho) / sqrt(hd.rho0) : 0.0;
+    out->solve_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - h->t_begin).count();
+    out->kernel_launches = h->launches;
+    return 0;
+}
+
 int sstep_cg_solve_end(sstep_cg_t* h, double* x, sstep_cg_result* out) {
     if (!h) return SSTEP_CG_ERR_ARG;
     if (!h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "solve_end: call solve_begin first");
@@ -1223,6 +1332,71 @@ int sstep_cg_solve_host(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rp
     if (rc < 0) return rc;
     CK(cudaMemcpyAsync(x, h->own_x, sizeof(double) * n, cudaMemcpyDeviceToHost, sm));
     CK(cudaStreamSynchronize(sm));
+    return rc;
+}
+
+// ---------------------------------------------------------------- measurement aid (measure.cuh)
+int sstep_cg_measure_bandwidth(sstep_cg_t* h, int variant, int64_t bytes, int passes, int reps, double* gbs_out) {
+    if (!h || !gbs_out || variant < 0 || variant > 3 || bytes < (1 << 20) || passes < 1 || reps < 1) return SSTEP_CG_ERR_ARG;
+    if (h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "measure_bandwidth: a solve is in progress");
+    CK(cudaSetDevice(h->device));
+    cudaStream_t sm = h->stream;
+    bytes &= ~(int64_t)4095;
+    unsigned char *src = nullptr, *dst = nullptr;
+    double* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = 0;
+    auto body = [&]() -> int {
+        CK(cudaMalloc(&src, (size_t)bytes));
+        CK(cudaMalloc(&sink, sizeof(double)));
+        CK(cudaMemsetAsync(src, 0, (size_t)bytes, sm));
+        if (variant == 2) {
+            CK(cudaMalloc(&dst, (size_t)bytes));
+            CK(cudaMemsetAsync(dst, 0, (size_t)bytes, sm));
+        }
+        CK(cudaEventCreate(&e0));
+        CK(cudaEventCreate(&e1));
+        constexpr int CH1 = 4096, D1 = 2, CH3 = 2048, D3 = 4;
+        const size_t smem1 = (size_t)8 * D1 * CH1 + 8 * D1 * 8, smem3 = (size_t)8 * D3 * CH3 + 8 * D3 * 8;
+        int occ = 1, grid = h->num_sms;
+        if (variant == 0) CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_ldg_kernel, 256, 0));
+        if (variant == 2) CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_copy_kernel, 256, 0));
+        if (variant == 1) {
+            CK(cudaFuncSetAttribute(measure_read_bulk_kernel<D1, CH1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_bulk_kernel<D1, CH1>, 256, smem1));
+        }
+        if (variant == 3) {
+            CK(cudaFuncSetAttribute(measure_read_bulk_kernel<D3, CH3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_bulk_kernel<D3, CH3>, 256, smem3));
+        }
+        grid = (occ < 1 ? 1 : occ) * h->num_sms;
+        double best = 0.0, sum = 0.0;
+        for (int rep = -1; rep < reps; rep++) {  // rep -1 = warm-up
+            CK(cudaEventRecord(e0, sm));
+            if (variant == 0) measure_read_ldg_kernel<<<grid, 256, 0, sm>>>((const double2*)src, bytes / 16, passes, sink);
+            else if (variant == 1) measure_read_bulk_kernel<D1, CH1><<<grid, 256, smem1, sm>>>(src, bytes / CH1, passes, sink);
+            else if (variant == 3) measure_read_bulk_kernel<D3, CH3><<<grid, 256, smem3, sm>>>(src, bytes / CH3, passes, sink);
+            else measure_copy_kernel<<<grid, 256, 0, sm>>>((const double2*)src, (double2*)dst, bytes / 16, passes);
+            CK(cudaGetLastError());
+            CK(cudaEventRecord(e1, sm));
+            CK(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep < 0) continue;
+            const double gbs = (variant == 2 ? 2.0 : 1.0) * (double)bytes * passes / (ms * 1e-3) / 1e9;
+            sum += gbs;
+            if (gbs > best) best = gbs;
+        }
+        gbs_out[0] = best;
+        gbs_out[1] = sum / reps;
+        return 0;
+    };
+    rc = body();
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (src) cudaFree(src);
+    if (dst) cudaFree(dst);
+    if (sink) cudaFree(sink);
     return rc;
 }
 
@@ -1345,7 +1519,18 @@ int sstep_cg_test_small_solve(sstep_cg_t* h, const double* M, const double* C, c
     if (!h || !M || !C || !m || !Wprev || !beta || !alpha || !W || !status_out) return SSTEP_CG_ERR_ARG;
     int rc = hook_prepare(h);
     if (rc) return rc;
-    small_solve_kernel<<<1, 32, 0, h->stream>>>(h->s, M, C, m, Wprev, beta, alpha, W, status_out);
+    small_solve_kernel<<<1, 32, 0, h->stream>>>(h->s, M, C, m, Wprev, nullptr, beta, alpha, W, nullptr, status_out);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
+int sstep_cg_test_small_solve_carried(sstep_cg_t* h, const double* M, const double* C, const double* m, const double* Lprev,
+                                      double* beta, double* alpha, double* W, double* Lout, int32_t* status_out) {
+    if (!h || !M || !C || !m || !Lprev || !beta || !alpha || !W || !Lout || !status_out) return SSTEP_CG_ERR_ARG;
+    int rc = hook_prepare(h);
+    if (rc) return rc;
+    small_solve_kernel<<<1, 32, 0, h->stream>>>(h->s, M, C, m, nullptr, Lprev, beta, alpha, W, Lout, status_out);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
     return 0;

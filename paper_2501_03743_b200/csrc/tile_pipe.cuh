@@ -51,6 +51,7 @@ __device__ __forceinline__ void tile_fill(int nseg, MakeSeg make_seg, uint64_t* 
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+    __syncwarp();  // the tail stores of the other lanes are ordered before lane 0's releasing arrive below
     if (lane == 0) {
         fence_proxy_async_smem();  // consumers' generic reads of this slot are ordered before the async writes
         mbar_expect_tx(full, bytes);  // one arrival + the transaction bytes (release: publishes the tail stores)

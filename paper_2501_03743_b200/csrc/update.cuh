@@ -226,6 +226,7 @@ init_kernel(int64_t n, const double* __restrict__ b, const double* __restrict__ 
         const double u = warp_sum_array(partials + gridDim.x, (int)gridDim.x, (int)threadIdx.x);
         for (int e = threadIdx.x; e < s * s; e += 32) {
             st->W[e] = (e / s == e % s) ? 1.0 : 0.0;  // W_prev = I with C = 0 gives beta = 0, W = M at k = 0
+            st->Lw[e] = (e / s == e % s) ? 1.0 : 0.0;  // its Cholesky factor (sqrt(1) = 1: the bits warp_cholesky gives)
             st->beta[e] = 0.0;
         }
         if (threadIdx.x == 0) {
@@ -250,7 +251,7 @@ __global__ void uniform_diag_kernel(int64_t n, const double* __restrict__ dinv, 
 }
 
 // ---- setup: dinv = 1/a_ii, structural validation, row-length statistics ----
-// err bits: 1 = rowptr not monotone / out of range, 2 = column index out of range, 4 = diagonal missing or <= 0
+// err bits: 1 = rowptr not monotone / out of range, 2 = column index out of range, 4 = diagonal missing, duplicated or <= 0
 __global__ void analyze_kernel(int64_t n, int64_t nnz, const int* __restrict__ rp, const int* __restrict__ ci,
                                const double* __restrict__ va, double* __restrict__ dinv, int* __restrict__ err,
                                int* __restrict__ max_len) {
@@ -260,15 +261,15 @@ __global__ void analyze_kernel(int64_t n, int64_t nnz, const int* __restrict__ r
         const int lo = rp[row], hi = rp[row + 1];
         if (lo < 0 || hi < lo || hi > nnz || (row == 0 && lo != 0) || (row == n - 1 && hi != nnz)) e |= 1;
         double d = 0.0;
-        bool found = false;
+        int found = 0;  // the diagonal entry must appear exactly once (the bulk SpMV takes 1/a_ii from the row itself)
         if (!e) {
             len = hi - lo;
             for (int k = lo; k < hi; k++) {
                 const int c = ci[k];
                 if (c < 0 || c >= n) e |= 2;
-                if (c == row) { d = va[k]; found = true; }
+                if (c == row) { d = va[k]; found++; }
             }
-            if (!found || !(d > 0.0)) e |= 4;
+            if (found != 1 || !(d > 0.0)) e |= 4;
         }
         dinv[row] = (e == 0) ? 1.0 / d : 0.0;
     }

@@ -36,19 +36,22 @@ def rel(a, b):
     return np.linalg.norm(a - b) / np.linalg.norm(b)
 
 
-CASES = [  # name, matrix, s, basis, block_rows, levels
-    ("p7_24_s4", lambda: gen.poisson7(24), 4, 0, 0, 0),                  # auto shape
-    ("p7_24_s4_b64", lambda: gen.poisson7(24), 4, 0, 64, 0),             # 216 blocks of 64 rows, lag 10: dependency stress
-    ("p7_24_s8_two_passes", lambda: gen.poisson7(24), 8, 0, 128, 3),     # passes of 3 + 3 + 2 levels
-    ("p7_40_s3_cheb", lambda: gen.poisson7(40), 3, 1, 2048, 0),          # Chebyshev epilogue reads R_{j-1}
-    ("p7_32_s2", lambda: gen.poisson7(32), 2, 0, 0, 0),
-    ("lap1d_s5", lambda: gen.poisson1d(4096), 5, 0, 32, 0),              # bandwidth 1: lag 2, 128 blocks
-    ("vc_16_s4", lambda: tuple(gen.make_config(5, N=16)[k] for k in ("rowptr", "colidx", "vals")), 4, 0, 0, 0),  # random order: bandwidth ~ n
+CASES = [  # name, matrix, s, basis, block_rows (0 = 512), levels per pass (0 = auto), slack in blocks (-1 = auto)
+    ("p7_24_s4", lambda: gen.poisson7(24), 4, 0, 0, 0, -1),                 # auto shape: 27 blocks of 512 rows
+    ("p7_24_s4_b64", lambda: gen.poisson7(24), 4, 0, 64, 0, 0),             # 216 blocks of 64 rows, no slack: every item waits
+    ("p7_24_s8_two_passes", lambda: gen.poisson7(24), 8, 0, 64, 3, 1),      # passes of 3 + 3 + 2 levels
+    ("p7_40_s3_cheb", lambda: gen.poisson7(40), 3, 1, 0, 0, -1),            # Chebyshev epilogue reads R_{j-1}
+    ("p7_40_s4_noslack", lambda: gen.poisson7(40), 4, 0, 0, 0, 0),          # 125 blocks of 512 rows, lag = dependency distance
+    ("p7_32_s2", lambda: gen.poisson7(32), 2, 0, 0, 0, -1),
+    ("p7_21_s3_ragged", lambda: gen.poisson7(21), 3, 0, 64, 0, 2),          # n = 9261 is not a multiple of 4: not applicable -> see below
+    ("lap1d_s5", lambda: gen.poisson1d(4096), 5, 0, 64, 0, 0),              # bandwidth 1, five levels in one pass
+    ("vc_16_s4", lambda: tuple(gen.make_config(5, N=16)[k] for k in ("rowptr", "colidx", "vals")), 4, 0, 0, 0, -1),  # random order: bandwidth ~ n
 ]
+CASES = [c for c in CASES if c[0] != "p7_21_s3_ragged"]
 
 
-@pytest.mark.parametrize("name,make,s,basis,block,levels", CASES, ids=[c[0] for c in CASES])
-def test_fused_mpk_matches_oracle_and_unfused(oracle_mod, cg_mod, torch_mod, name, make, s, basis, block, levels):
+@pytest.mark.parametrize("name,make,s,basis,block,levels,slack", CASES, ids=[c[0] for c in CASES])
+def test_fused_mpk_matches_oracle_and_unfused(oracle_mod, cg_mod, torch_mod, name, make, s, basis, block, levels, slack):
     import scipy.sparse as sp
     rp, ci, v = make()[:3]
     n = rp.size - 1
@@ -56,11 +59,12 @@ def test_fused_mpk_matches_oracle_and_unfused(oracle_mod, cg_mod, torch_mod, nam
     dinv = oracle_mod.dinv(rp, ci, v)
     absA = sp.csr_matrix((np.abs(v), ci, rp), shape=(n, n))
     t = lambda a: dev(torch_mod, a)
-    with cg_mod.SStepCG(0, mpk_fused=2, basis=basis, mpk_block_rows=block, mpk_levels=levels) as h:
+    with cg_mod.SStepCG(0, mpk_fused=2, basis=basis, mpk_block_rows=block, mpk_levels=levels, mpk_slack=slack) as h:
         h.setup(t(rp), t(ci), t(v), s)
         assert h.get_info("mpk_fused") == 1
-        if block:
-            assert h.get_info("mpk_block_rows") == block
+        assert h.get_info("mpk_block_rows") == (block or 512)
+        if slack >= 0:
+            assert h.get_info("mpk_lag") == h.get_info("mpk_lag_dep") + slack
         R, AR = (a.cpu().numpy() for a in h.test_mpk(t(r)))
         for _ in range(3):                                   # reproducible whatever the arrival order of the warps
             R2, AR2 = (a.cpu().numpy() for a in h.test_mpk(t(r)))
@@ -91,7 +95,7 @@ def test_solver_on_fused_mpk_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg, 
     rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
     basis = 1 if s == 8 else 0
     ref = oracle_mod.sstep(rp, ci, v, b, s, rtol=c["rtol"], maxit=c["maxit"], basis=basis, xhist_cap=3)
-    with cg_mod.SStepCG(0, mpk_fused=2, resident=1, basis=basis, mpk_block_rows=1024) as h:
+    with cg_mod.SStepCG(0, mpk_fused=2, resident=1, basis=basis, mpk_block_rows=64 if N == 40 else 0) as h:
         h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), s)
         assert h.get_info("mpk_fused") == 1
         kpo = h.get_info("kernels_per_outer")
@@ -113,7 +117,7 @@ def test_solver_on_fused_mpk_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg, 
 def test_fused_mpk_selection(cg_mod, torch_mod):
     t = lambda a: dev(torch_mod, a)
     rp, ci, v = gen.poisson7(64)                     # 262 144 rows, half bandwidth 4096
-    with cg_mod.SStepCG(0, resident=1) as h:         # experimental: never chosen automatically
+    with cg_mod.SStepCG(0, resident=1) as h:         # auto: only for matrices much larger than L2
         h.setup(t(rp), t(ci), t(v), 4)
         assert h.get_info("mpk_fused") == 0
     with cg_mod.SStepCG(0, resident=1, mpk_fused=2) as h:
@@ -123,9 +127,9 @@ def test_fused_mpk_selection(cg_mod, torch_mod):
         assert h.get_info("mpk_lag") >= h.get_info("mpk_lag_dep")
     for opts, s in ((dict(form=1), 4), (dict(), 1)):  # moment form (its SpMV epilogues carry the moments), s = 1: not applicable
         with cg_mod.SStepCG(0, mpk_fused=2, **opts) as h:
-            with pytest.raises(cg_mod.SStepCGError, match="fused matrix-powers"):
+            with pytest.raises(cg_mod.SStepCGError, match="matrix-powers"):
                 h.setup(t(rp), t(ci), t(v), s)
     rp, ci, v = gen.poisson27(12)                    # several lanes per row: not the thread-per-row shape
     with cg_mod.SStepCG(0, mpk_fused=2) as h:
-        with pytest.raises(cg_mod.SStepCGError, match="fused matrix-powers"):
+        with pytest.raises(cg_mod.SStepCGError, match="matrix-powers"):
             h.setup(t(rp), t(ci), t(v), 4)

@@ -185,6 +185,47 @@ def test_edge_cases(oracle_mod, cg_mod, torch_mod):
     assert res["status"] == 0 and abs(x[0] - 0.5) <= 1e-15
 
 
+def test_x_may_alias_x0_and_peek_reports_history(oracle_mod, cg_mod, torch_mod):
+    """include/sstep_cg.h: "`x` ... may alias x0" -- sstep_cg_solve called with the SAME device buffer for x0 and x, on
+    the graph path and on the resident path; and sstep_cg_solve_peek after every outer iteration gives the oracle's
+    relative-residual history (Alg. 3 l.31-33)."""
+    c = gen.make_config(1, N=12)
+    x0 = np.random.default_rng(19).uniform(-1, 1, c["n"])
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 2, x0=x0, rtol=1e-9, maxit=500, history=True)
+    t = lambda a: torch_mod.from_numpy(np.ascontiguousarray(a)).cuda()
+    for resident in (1, 0):
+        with cg_mod.SStepCG(0, resident=resident) as h:
+            h.setup(t(c["rowptr"]), t(c["colidx"]), t(c["vals"]), 2)
+            buf = t(x0)
+            x, res = h.solve(t(c["b"]), x0=buf, rtol=1e-9, maxit=500, out=buf)
+            assert x.data_ptr() == buf.data_ptr()
+            assert res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
+            assert rel(buf.cpu().numpy(), ref["x"]) <= 1e-8 or res["outer_iters"] != ref["iters"]
+            assert rel(buf.cpu().numpy(), c["xstar"]) <= 1e-7
+            h.solve_begin(t(c["b"]), t(x0), 1e-9)
+            hist = []
+            for _ in range(500):
+                h.iterate(1)
+                p = h.solve_peek()
+                hist.append(p["relres"])
+                if p["status"] != -1:
+                    break
+            _, res2 = h.solve_end()
+            assert res2["outer_iters"] == len(hist) == res["outer_iters"]
+            k = min(len(hist), ref["iters"]) // 2
+            assert np.allclose(hist[:k], ref["hist"][:k], rtol=1e-6, atol=0)
+
+
+def test_measure_bandwidth_runs(cg_mod, torch_mod):
+    """The measurement aid of bench.py's read-side peak: every variant returns a positive, plausible figure."""
+    with cg_mod.SStepCG(0) as h:
+        for variant in (0, 1, 2, 3):
+            best, mean = h.measure_bandwidth(variant, 256 << 20, passes=1, reps=3)
+            assert 100.0 < mean <= best < 20000.0, (variant, best, mean)
+        best, _ = h.measure_bandwidth(0, 32 << 20, passes=20, reps=3)      # L2-resident sweep
+        assert best > 100.0
+
+
 def test_rank_deficient_block_reports_breakdown(oracle_mod, cg_mod, torch_mod):
     """Degenerate case of the method (see test_oracle_solvers.test_rank_deficient_last_block)."""
     rp, ci, v = gen.poisson1d(64)
