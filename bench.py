@@ -287,13 +287,19 @@ def run_ours(args):
                 if args.read_peak:
                     big = 8 << 30
                     rp_ldg = h.measure_bandwidth(0, big, 1, 5)
-                    rp_bulk = max(h.measure_bandwidth(1, big, 1, 5), h.measure_bandwidth(3, big, 1, 5))
+                    # bulk-copy path by the number of copies an SM keeps in flight (variants 3, 1, 5, 4 = 96, 48, 32, 24): HBM and L2
+                    inflight = {96: 3, 48: 1, 32: 5, 24: 4}
+                    bulk_hbm = {k: h.measure_bandwidth(v, big, 1, 3)[0] for k, v in inflight.items()}
+                    bulk_l2 = {k: h.measure_bandwidth(v, 48 << 20, 64, 3)[0] for k, v in inflight.items()}
+                    rp_bulk = max(bulk_hbm.values())
                     cp = h.measure_bandwidth(2, big // 2, 1, 5)
-                    l2 = max(h.measure_bandwidth(0, 48 << 20, 64, 5), h.measure_bandwidth(1, 48 << 20, 64, 5))
-                    read_peak = dict(read_ldg_gbs=rp_ldg[0], read_bulk_gbs=rp_bulk[0], read_peak_gbs=max(rp_ldg[0], rp_bulk[0]),
-                                     copy_gbs=cp[0], l2_read_48mb_gbs=l2[0], mean=dict(read_ldg=rp_ldg[1], read_bulk=rp_bulk[1], copy=cp[1], l2=l2[1]),
+                    l2 = h.measure_bandwidth(0, 48 << 20, 64, 5)
+                    read_peak = dict(read_ldg_gbs=rp_ldg[0], read_bulk_gbs=rp_bulk, read_peak_gbs=max(rp_ldg[0], rp_bulk),
+                                     copy_gbs=cp[0], l2_read_48mb_gbs=max(l2[0], max(bulk_l2.values())),
+                                     bulk_by_copies_in_flight_per_sm=dict(hbm_gbs=bulk_hbm, l2_gbs=bulk_l2),
+                                     mean=dict(read_ldg=rp_ldg[1], copy=cp[1], l2_ldg=l2[1]),
                                      how="sstep_cg_measure_bandwidth: 8 GiB zero-filled buffer read once per launch (copy: 4 GiB "
-                                         "read + 4 GiB written), best / mean of 5 launches; l2 = a 48 MiB buffer read 64 times in one launch")
+                                         "read + 4 GiB written), best / mean of 3-5 launches; l2 = a 48 MiB buffer read 64 times in one launch")
             else:
                 ms, launches, res = time_outer_iterations(torch, h, b, s, args.steps, args.warmup, barrier)
             agg = aggregate_replicas(ms, args.steps, world, reduce_max)

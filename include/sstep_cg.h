@@ -95,7 +95,7 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *   "spmv_variant" 0 auto (default) | 1 force the generic vector-per-row kernel | 2 force the bulk-staged kernel with
  *                  per-warp rings | 3 force the CTA-pipelined bulk-staged kernel (thread-per-row matrices; auto picks it
  *                  there: few large bulk copies in flight per SM instead of many small ones)
- *   "spmv_cta_depth" 2 | 3 (default) | 4 stages of the CTA-pipelined SpMV's ring; "spmv_cta_per_sm" 2 | 3 (default) CTAs per SM
+ *   "spmv_cta_depth" 2 (default) | 3 | 4 stages of the CTA-pipelined SpMV's ring; "spmv_cta_per_sm" 2 | 3 (default) CTAs per SM
  *   "lanes"        0 auto | 1,2,4,8,16,32 lanes per row
  *   "spmv_depth"   2 (default) | 3 | 4 slots of the bulk-staged SpMV's per-warp shared-memory ring
  *   "block_variant" 0 auto (default: Gram/update through the TMA tile pipeline for s >= 5, register kernels below)
@@ -127,18 +127,6 @@ int sstep_cg_setup(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *ro
  *                  stop test, direction update): the classical two-reduction comparator.  Needs s = 1 at setup;
  *                  "outer iterations" are then CG iterations.  (The paper's one-reduction baseline "fcg", Alg. 2, is
  *                  method 0 with s = 1.)
- *   "mpk_fused"    0 auto | 1 off | 2 force.  Wavefront-ordered matrix-powers kernel (csrc/mpk_wave.cuh): the s SpMVs of
- *                  Alg. 4 run as ONE kernel per pass of g levels whose levels follow each other down a banded matrix a
- *                  fixed distance apart, so that the CSR arrays (and the basis vectors) are re-read from L2 instead of
- *                  HBM: persistent CTAs claim work items (level, block of 512 rows) in wavefront order with one atomic
- *                  each; per-item done flags + per-level watermarks carry the dependencies.  Applies to thread-per-row
- *                  matrices on the CTA-pipelined SpMV (7-point configs) with s >= 2, form = 0, n % 4 == 0 and 16-byte
- *                  aligned rowptr; bitwise the same results as the separate SpMVs.  Hardware assumption (stated in the
- *                  file header): the gathers of a column written by other SMs in the same launch go through L1 without an
- *                  acquire -- no sector can be cached before it is final, and the writers publish with a gpu-scope release.
- *                  "mpk_levels" (levels per pass, 0 = as many as keep the re-read window inside L2), "mpk_slack" (blocks a
- *                  level trails its predecessor by beyond the dependency distance, -1 = auto) and "mpk_block_rows"
- *                  (0 = 512 | 64: small items for dependency tests on small matrices) override the shape.
  *   "pdl"          1 (default) | 0.  Programmatic dependent launch: the kernels of one outer iteration (a1 x s, a2 + a3, a4)
  *                  carry the programmatic-stream-serialization attribute, captured as programmatic edges of the graph, so
  *                  the next kernel's blocks become resident while the current one drains (the SpMV also stages its first
@@ -185,11 +173,13 @@ int sstep_cg_solve_host(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_
 int sstep_cg_profile_outer(sstep_cg_t *handle, int reps, double *ms_host);
 
 /* Measurement aid (bench.py's read-side peak): stream a private zero-filled buffer of `bytes` bytes (>= 1 MiB, rounded
- * down to 4 KiB) `passes` times inside one launch with hand-written kernels that use the hot path's own load
+ * down to 8 KiB) `passes` times inside one launch with hand-written kernels that use the hot path's own load
  * instructions, `reps` timed launches after one warm-up (CUDA events on the solver's stream):
  *   variant 0  128-bit ld.global.nc.L1::no_allocate reads     (Gram / update kernels' loads)
- *   variant 1  cp.async.bulk reads, 2 x 4 KiB ring per warp   (bulk-staged SpMV's loads)
- *   variant 3  cp.async.bulk reads, 4 x 2 KiB ring per warp
+ *   variant 1  cp.async.bulk reads, 24 warps x 2 x 4 KiB per SM: 48 bulk copies in flight per SM
+ *   variant 3  cp.async.bulk reads, 24 warps x 4 x 2 KiB: 96 in flight (the shape of round 1's per-warp SpMV rings)
+ *   variant 4  cp.async.bulk reads, 12 warps x 2 x 8 KiB: 24 in flight
+ *   variant 5  cp.async.bulk reads, 16 warps x 2 x 4 KiB: 32 in flight (the bulk path is at full speed up to ~32)
  *   variant 2  128-bit copy; read + written bytes both counted (comparable with MEASURED_PEAKS.json hbm_gbs)
  * gbs_out_host[0] = best, [1] = mean GB/s.  bytes >> L2 with passes = 1 gives the HBM figure; a buffer that fits L2
  * with passes > 1 gives the L2-hit bandwidth.  Not allowed during a solve. */

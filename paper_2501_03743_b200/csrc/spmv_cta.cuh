@@ -19,6 +19,65 @@
 #include "common.cuh"
 #include "spmv.cuh"
 
+// One row per lane out of a staged tile: acc = sum_k a_k x[col_k] over the row's entries [lo, hi) (sv / sc = the stage's
+// vals / cols, pre-offset so that they are indexed by the global nnz index), the fragment of <= 8 entries summed in
+// ascending order, then the remainder of longer rows -- the order of spmv_bulk_kernel at L = 1, bit for bit.
+// Lean on purpose (the SpMV issues ~230 instructions per 32 rows and runs at ~50 % issue utilisation, which is what
+// bounds a level served from L2): entries past the row's end re-read the row's FIRST entry with the value masked to
+// zero, so that the index and the gather need no predicate (the gathered column is a genuine neighbour of this row,
+// hence a valid index whose x cannot be non-finite unless the row's true result already is); `lo` must be a staged
+// index also for empty / dead rows.  Two phases, so that the caller can hand the stage back between them.  UNI: the diagonal is constant (every Poisson config), 1 / a_ii is a kernel argument
+// and the pick-up of a_ii from the row disappears; else diag returns the row's own diagonal entry.
+struct StageRowFrag {
+    double v[8], xv[8];
+    double rem, diag;
+};
+// phase 1: fragment to registers, gathers issued (after it the stage may be handed back)
+template <bool UNI>
+__device__ __forceinline__ void stage_row_load(const double* sv, const int* sc, int lo, int hi, int row,
+                                               const double* __restrict__ x, StageRowFrag& f) {
+    constexpr int U = 8;
+    int c[U];
+    f.diag = 0.0;
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const int kk = lo + u;
+        const bool ok = kk < hi;
+        const int k2 = ok ? kk : lo;
+        c[u] = sc[k2];
+        const double t = sv[k2];
+        f.v[u] = ok ? t : 0.0;
+        if (!UNI) { if (ok && c[u] == row) f.diag = t; }
+    }
+#pragma unroll
+    for (int u = 0; u < U; u++) f.xv[u] = x[c[u]];
+    double rem = 0.0;
+    for (int k0 = lo + U; k0 < hi; k0 += U) {  // rows longer than U entries: further batches
+        int cc[U];
+        double vv[U], xx[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int kk = k0 + u;
+            const bool ok = kk < hi;
+            cc[u] = ok ? sc[kk] : -1;
+            vv[u] = ok ? sv[kk] : 0.0;
+            if (!UNI) { if (cc[u] == row) f.diag = vv[u]; }
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) xx[u] = (cc[u] >= 0) ? x[cc[u]] : 0.0;
+#pragma unroll
+        for (int u = 0; u < U; u++) rem = fma(vv[u], xx[u], rem);
+    }
+    f.rem = rem;
+}
+// phase 2: the row sum (waits for the gathers)
+__device__ __forceinline__ double stage_row_sum(const StageRowFrag& f) {
+    double acc = 0.0;
+#pragma unroll
+    for (int u = 0; u < 8; u++) acc = fma(f.v[u], f.xv[u], acc);
+    return acc + f.rem;
+}
+
 template <int D, int TR, int CAPT>
 struct SpmvCtaCfg {
     static constexpr int NCW = TR / 32;                 // consumer warps
@@ -28,14 +87,14 @@ struct SpmvCtaCfg {
     static_assert(CAPT % 4 == 0 && TR % 32 == 0, "stage sub-buffers must stay 16-byte aligned");
 };
 
-template <int D, int TR, int CAPT, bool MOM, int MINB>
+template <int D, int TR, int CAPT, bool MOM, int MINB, bool UNI>
 __global__ void __launch_bounds__(TR + 32, MINB)
 spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restrict__ ci, const double* __restrict__ va,
                 const double* __restrict__ x, double* __restrict__ y, double* __restrict__ yjac,
                 const double* __restrict__ xprev, int mode, const ScgState* __restrict__ st, int num_tiles,
-                double* __restrict__ mom_a, double* __restrict__ mom_b) {
+                double* __restrict__ mom_a, double* __restrict__ mom_b, double dinv_uniform) {
     using Cfg = SpmvCtaCfg<D, TR, CAPT>;
-    constexpr int NCW = Cfg::NCW, U = 8;
+    constexpr int NCW = Cfg::NCW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* svals = reinterpret_cast<double*>(smem_raw);                                  // [D][CAPT]
     int* scols = reinterpret_cast<int*>(smem_raw + (size_t)D * CAPT * sizeof(double));    // [D][CAPT]
@@ -131,52 +190,23 @@ spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restric
         const int a0 = s_a0[sl];
         const double* sv = svals + (size_t)sl * CAPT - a0;
         const int* sc = scols + (size_t)sl * CAPT - a0;
-        int c[U];
-        double v[U], xv[U];
-        double diag = 0.0;
-#pragma unroll
-        for (int u = 0; u < U; u++) {
-            const int kk = lo + u;
-            const bool ok = kk < hi;
-            c[u] = ok ? sc[kk] : -1;
-            v[u] = ok ? sv[kk] : 0.0;
-            if (c[u] == row) diag = v[u];
-        }
-#pragma unroll
-        for (int u = 0; u < U; u++) xv[u] = (c[u] >= 0) ? x[c[u]] : 0.0;
+        const bool live = row < n;
+        StageRowFrag f;
+        stage_row_load<UNI>(sv, sc, live ? lo : a0, live ? hi : a0, row, x, f);
         double xrow = 0.0, xpv = 0.0;
-        if ((MOM || (jac && mode != 0)) && row < n) {
+        if ((MOM || (jac && mode != 0)) && live) {
             xrow = x[row];
             if (mode == 2) xpv = xprev[row];
         }
-        double rem = 0.0;
-        for (int k0 = lo + U; k0 < hi; k0 += U) {  // rows longer than U entries: further batches
-            int cc[U];
-            double vv[U], xx[U];
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const int kk = k0 + u;
-                const bool ok = kk < hi;
-                cc[u] = ok ? sc[kk] : -1;
-                vv[u] = ok ? sv[kk] : 0.0;
-                if (cc[u] == row) diag = vv[u];
-            }
-#pragma unroll
-            for (int u = 0; u < U; u++) xx[u] = (cc[u] >= 0) ? x[cc[u]] : 0.0;
-#pragma unroll
-            for (int u = 0; u < U; u++) rem = fma(vv[u], xx[u], rem);
-        }
         __syncwarp();  // every lane has read the stage
         if (lane == 0) mbar_arrive(&empty[sl]);
-        double acc = 0.0;
-#pragma unroll
-        for (int u = 0; u < U; u++) acc = fma(v[u], xv[u], acc);
-        acc += rem;
-        if (row < n) {
+        const double acc = stage_row_sum(f);
+        const double diag = f.diag;
+        if (live) {
             y[row] = acc;
             if (MOM) ma = fma(xrow, acc, ma);
             if (jac) {
-                double z = __drcp_rn(diag) * acc;
+                double z = (UNI ? dinv_uniform : __drcp_rn(diag)) * acc;
                 if (MOM) mb = fma(z, acc, mb);
                 if (mode == 1) z = z - xrow;
                 else if (mode == 2) z = 2.0 * (z - xrow) - xpv;

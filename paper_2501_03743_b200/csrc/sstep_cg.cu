@@ -12,7 +12,6 @@
 #include "gram_tma.cuh"
 #include "measure.cuh"
 #include "moment.cuh"
-#include "mpk_wave.cuh"
 #include "pcg.cuh"
 #include "reorder.cuh"
 #include "resident.cuh"
@@ -43,10 +42,6 @@ constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D
 // CTA-pipelined SpMV (spmv_cta.cuh), thread-per-row matrices: tiles of 256 rows, stage capacity 1800 entries (a 7-point
 // tile holds <= 1792; three stages x three CTAs = 194 KB of shared memory per SM, ~33 KB left for L1)
 constexpr int CTA_TR = 256, CTA_CAPT = 1800;
-// wavefront matrix-powers kernel (mpk_wave.cuh): ring stages, stages per work item (item = MW_SPI * CTA_TR rows), most levels per pass
-constexpr int MW_D = 2, MW_SPI = 2, MW_MAXLEV = 5;
-constexpr int MW_SMALL_TR = 64, MW_SMALL_CAPT = 520;  // option mpk_block_rows = 64: items of 64 rows (rows of <= 8 entries)
-constexpr bool MW_AUTO = false;  // (selected automatically only once it beats the separate SpMVs)
 
 }  // namespace
 
@@ -56,7 +51,7 @@ struct sstep_cg {
     cudaStream_t cap_stream = nullptr;  // owned, used only to capture the graph
     int num_sms = 0;
     // options
-    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0, mpk_fused_opt = 0, mpk_block_opt = 0, mpk_levels_opt = 0, mpk_slack_opt = -1, pdl = 1;
+    int basis = 0, spmv_variant = 0, lanes_opt = 0, use_graph = 1, spmv_depth = 2, block_variant = 0, form = 0, resident_opt = 0, reorder_opt = 0, replace_every = 0, method = 0, pdl = 1;
     // problem (borrowed CSR)
     int64_t n = 0, nnz = 0;
     int s = 0;
@@ -80,7 +75,7 @@ struct sstep_cg {
     bool bulk = false;
     int bulk_cap = 256, bulk_wpc = 8;
     bool cta = false;             // thread-per-row matrices: CTA-pipelined SpMV (spmv_cta.cuh) instead of the per-warp rings
-    int cta_depth = 3, cta_minb = 3, cta_tiles = 0;
+    int cta_depth = 2, cta_minb = 3, cta_tiles = 0;
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0, pcg_grid = 0;
     bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
@@ -94,11 +89,6 @@ struct sstep_cg {
     int *own_prp = nullptr, *own_pci = nullptr;
     double *own_pva = nullptr, *bperm = nullptr, *x0perm = nullptr;
     int cm_levels = 0, cm_comps = 0, far_permille = 0;
-    // wavefront-fused matrix-powers kernel (mpk_wave.cuh): the CSR arrays are read from HBM once per pass of `mw_levels` levels
-    bool mpk_fused = false;
-    int bandwidth = 0, mw_block = 0, mw_nb = 0, mw_lag = 0, mw_lag_dep = 0, mw_levels = 0, mw_grid = 0;
-    size_t mw_sync_ints = 0;
-    int* mw_sync = nullptr;  // [s * nb] done counters, then [s] watermarks
     // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
     bool resident = false;
     int res_grid = 0, res_rpb = 0, res_nzcap = 0, res_threads = 0;
@@ -172,23 +162,27 @@ bulk_fn_t bulk_kernel_for(int depth, bool mom, int cap) {
     return mom ? bulk_kernel_mom<L, true>(depth) : bulk_kernel_mom<L, false>(depth);
 }
 
-template <bool MOM>
-bulk_fn_t cta_kernel_mom(int depth, int minb) {
+using cta_fn_t = void (*)(int, int, const int*, const int*, const double*, const double*, double*, double*,
+                          const double*, int, const ScgState*, int, double*, double*, double);
+template <bool MOM, bool UNI>
+cta_fn_t cta_kernel_mu(int depth, int minb) {
     if (minb == 2) {
         switch (depth) {
-            case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 2>;
-            case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 2>;
-            default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 2>;
+            case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 2, UNI>;
+            case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 2, UNI>;
+            default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 2, UNI>;
         }
     }
     switch (depth) {
-        case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 3>;
-        case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 3>;
-        default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 3>;
+        case 2: return spmv_cta_kernel<2, CTA_TR, CTA_CAPT, MOM, 3, UNI>;
+        case 3: return spmv_cta_kernel<3, CTA_TR, CTA_CAPT, MOM, 3, UNI>;
+        default: return spmv_cta_kernel<4, CTA_TR, CTA_CAPT, MOM, 3, UNI>;
     }
 }
-bulk_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
-    return mom ? cta_kernel_mom<true>(h->cta_depth, h->cta_minb) : cta_kernel_mom<false>(h->cta_depth, h->cta_minb);
+cta_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
+    const bool uni = h->dinv_uniform > 0.0;
+    if (mom) return uni ? cta_kernel_mu<true, true>(h->cta_depth, h->cta_minb) : cta_kernel_mu<true, false>(h->cta_depth, h->cta_minb);
+    return uni ? cta_kernel_mu<false, true>(h->cta_depth, h->cta_minb) : cta_kernel_mu<false, false>(h->cta_depth, h->cta_minb);
 }
 size_t cta_smem_for(int depth) { return (size_t)depth * CTA_CAPT * 12 + (size_t)depth * 24; }
 
@@ -197,7 +191,7 @@ cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double*
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if (L == 1 && h->cta) {
         return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, CTA_TR + 32, cta_smem_for(h->cta_depth), sm, (int)h->n,
-                        (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->cta_tiles, mom_a, mom_b);
+                        (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->cta_tiles, mom_a, mom_b, h->dinv_uniform);
     }
     if (h->bulk) {
         return launch_k(h, bulk_kernel_for<L>(h->spmv_depth, mom_a != nullptr, h->bulk_cap), h->spmv_grid, h->bulk_wpc * 32,
@@ -415,27 +409,6 @@ cudaError_t resident_op(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ
 // Alg. 4 on the given buffers: s Jacobi-fused SpMVs (R(:,1) must already hold D^-1 r)
 cudaError_t launch_mpk(sstep_cg* h, cudaStream_t sm, double* R, double* AR, const ScgState* st) {
     const int64_t n = h->n;
-    if (h->mpk_fused) {  // wavefront order: one launch per pass of mw_levels levels (mpk_wave.cuh)
-        for (int j0 = 0; j0 < h->s; j0 += h->mw_levels) {
-            cudaError_t e = cudaMemsetAsync(h->mw_sync, 0, sizeof(int) * h->mw_sync_ints, sm);
-            if (e != cudaSuccess) return e;
-            MpkWaveParams p;
-            p.n = (int)n; p.nnz = (int)h->nnz; p.s = h->s;
-            p.j0 = j0; p.nlev = (h->s - j0 < h->mw_levels) ? h->s - j0 : h->mw_levels;
-            p.nb = h->mw_nb; p.lag = h->mw_lag; p.dep = h->mw_lag_dep; p.bp = h->mw_lag - h->mw_lag_dep; p.basis = h->basis;
-            p.rp = h->rp; p.ci = h->ci; p.va = h->va; p.R = R; p.AR = AR; p.st = st;
-            p.watermark = h->mw_sync; p.done = h->mw_sync + 32 * MW_MAXLEV;
-            if (h->mw_block == MW_SMALL_TR)  // (64-row items: dependency stress on small matrices, tests only)
-                e = launch_k(h, mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, h->mw_grid, MW_SMALL_TR + 32,
-                             MpkWaveCfg<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>::SMEM, sm, p);
-            else
-                e = launch_k(h, mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, h->mw_grid, CTA_TR + 32,
-                             MpkWaveCfg<MW_D, CTA_TR, CTA_CAPT, MW_SPI>::SMEM, sm, p);
-            if (e != cudaSuccess) return e;
-            h->launches++;
-        }
-        return cudaSuccess;
-    }
     for (int j = 0; j < h->s; j++) {
         double* yjac = (j + 1 < h->s) ? R + (int64_t)(j + 1) * n : nullptr;
         int mode = 0;
@@ -494,7 +467,7 @@ void free_problem(sstep_cg* h) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
-    int** ibufs[] = {&h->perm, &h->rank, &h->own_prp, &h->own_pci, &h->mw_sync};
+    int** ibufs[] = {&h->perm, &h->rank, &h->own_prp, &h->own_pci};
     for (int** b : ibufs) {
         if (*b) cudaFree(*b);
         *b = nullptr;
@@ -521,22 +494,7 @@ void free_owned(sstep_cg* h) {
 
 int kernels_per_outer(const sstep_cg* h) {
     if (h->method == 1) return 3;
-    if (h->mpk_fused) return (h->s + h->mw_levels - 1) / h->mw_levels + 2;
     return h->s + 2;
-}
-
-// half bandwidth in rows: max |col - row|
-__global__ void bandwidth_kernel(int64_t n, const int* __restrict__ rp, const int* __restrict__ ci, int* __restrict__ out) {
-    const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int m = 0;
-    if (row < n)
-        for (int k = rp[row]; k < rp[row + 1]; k++) {
-            const int64_t d = (int64_t)ci[k] - row;
-            m = max(m, (int)(d < 0 ? -d : d));
-        }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
 }
 
 __global__ void iota_kernel(int64_t n, int* __restrict__ p) {
@@ -741,79 +699,6 @@ int setup_block_kernels(sstep_cg* h) {
     return 0;
 }
 
-// shape of the wavefront-ordered matrix-powers kernel (mpk_wave.cuh)
-int setup_mpk_wave(sstep_cg* h) {
-    const int64_t n = h->n;
-    const int64_t nnz = h->nnz;
-    const int s = h->s;
-    cudaStream_t sm = h->stream;
-    int hs[4] = {0, 0, 0, 0};
-    h->mpk_fused = false;
-    h->mw_levels = 0;
-    // thread-per-row matrices on the CTA-pipelined SpMV shape, Gram form, s >= 2, n % 4 == 0 (32-byte aligned columns of
-    // R), 16-byte aligned rowptr, and a bandwidth whose re-read window fits the fast part of L2.  Auto: only when the
-    // matrix is much larger than L2 (otherwise the separate SpMVs already re-read it from L2)
-    const bool applicable = h->cta && h->form == 0 && h->method == 0 && s >= 2 && n % 4 == 0 && (((uintptr_t)h->rp) & 15) == 0;
-    const bool wanted = h->mpk_fused_opt == 2 || (MW_AUTO && h->mpk_fused_opt == 0 && 12.0 * (double)nnz > 400.0e6);
-    if (applicable && wanted) {
-        CK(cudaMemsetAsync(h->iscratch + 3, 0, sizeof(int), sm));
-        bandwidth_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(n, h->rp, h->ci, h->iscratch + 3);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(hs + 3, h->iscratch + 3, sizeof(int), cudaMemcpyDeviceToHost, sm));
-        CK(cudaStreamSynchronize(sm));
-        h->bandwidth = hs[3];
-        using WC = MpkWaveCfg<MW_D, CTA_TR, CTA_CAPT, MW_SPI>;
-        using WS = MpkWaveCfg<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>;
-        const bool small = h->mpk_block_opt == MW_SMALL_TR && h->max_row_len <= 8;
-        int occ = 0;
-        if (small) {
-            CK(cudaFuncSetAttribute(mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WS::SMEM));
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<MW_D, MW_SMALL_TR, MW_SMALL_CAPT, 1>, WS::THREADS, WS::SMEM));
-        } else {
-            CK(cudaFuncSetAttribute(mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WC::SMEM));
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mpk_wave_kernel<MW_D, CTA_TR, CTA_CAPT, MW_SPI>, WC::THREADS, WC::SMEM));
-        }
-        if (occ > 3) occ = 3;
-        if (occ >= 1) {
-            const int64_t B = small ? WS::BR : WC::BR;
-            const int64_t nb = (n + B - 1) / B;
-            const int64_t grid = (int64_t)occ * h->num_sms < nb ? (int64_t)occ * h->num_sms : nb;
-            const int64_t dep = (h->bandwidth + B - 1) / B + 1;
-            const double row_bytes = 12.0 * (double)nnz / (double)n + 4.0 + 24.0;
-            // levels per pass: the largest g whose re-read window (g - 1) * lag blocks stays within ~56 MB of L2; the slack
-            // covers the items the grid has in flight (about one per CTA and level)
-            int g = s < MW_MAXLEV ? s : MW_MAXLEV;
-            if (h->mpk_levels_opt) g = h->mpk_levels_opt < g ? h->mpk_levels_opt : g;
-            int64_t slack = 0, lag = 0;
-            for (;; g--) {
-                slack = (2 * grid) / (g > 1 ? g : 1) + 8;
-                if (h->mpk_slack_opt >= 0) slack = h->mpk_slack_opt;
-                lag = dep + slack;
-                if (g <= 2 || h->mpk_levels_opt || ((double)(g - 1) * (double)lag + (double)slack) * (double)B * row_bytes <= 56.0e6) break;
-            }
-            const bool fits = ((double)(g - 1) * (double)lag + (double)slack) * (double)B * row_bytes <= 80.0e6;
-            if (g >= 2 && (fits || h->mpk_fused_opt == 2) && (nb + (int64_t)(g - 1) * lag) * g < (int64_t(1) << 31)) {
-                const int passes = (s + g - 1) / g;
-                h->mw_levels = (s + passes - 1) / passes;
-                h->mw_block = (int)B;
-                h->mw_nb = (int)nb;
-                h->mw_lag = (int)lag;
-                h->mw_lag_dep = (int)dep;
-                h->mw_grid = (int)grid;
-                h->mw_sync_ints = 32 * (size_t)MW_MAXLEV + (size_t)MW_MAXLEV * nb;
-                CK(cudaMalloc(&h->mw_sync, sizeof(int) * h->mw_sync_ints));
-                h->mpk_fused = true;
-            }
-        }
-    }
-    if (h->mpk_fused_opt == 2 && !h->mpk_fused) {
-        free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: wavefront matrix-powers kernel forced but not applicable (needs the CTA-pipelined "
-                                         "thread-per-row SpMV, s >= 2, form = 0, n % 4 == 0, 16-byte aligned rowptr)");
-    }
-    return 0;
-}
-
 // eligibility and shape of the resident (whole loop in one cooperative launch) path
 int setup_resident(sstep_cg* h) {
     const int64_t n = h->n;
@@ -983,10 +868,6 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
     else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
     else if (k == "method" && (value == 0 || value == 1)) h->method = (int)value;
-    else if (k == "mpk_fused" && value >= 0 && value <= 2) h->mpk_fused_opt = (int)value;
-    else if (k == "mpk_block_rows" && (value == 0 || value == MW_SMALL_TR)) h->mpk_block_opt = (int)value;
-    else if (k == "mpk_levels" && value >= 0 && value <= SSTEP_CG_SMAX) h->mpk_levels_opt = (int)value;
-    else if (k == "mpk_slack" && value >= -1 && value <= (1 << 20)) h->mpk_slack_opt = (int)value;
     else if (k == "pdl" && (value == 0 || value == 1)) h->pdl = (int)value;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown option or bad value: " + k);
     return 0;
@@ -1019,14 +900,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "replace_every") *value = h->replace_every;
     else if (k == "method") *value = h->method;
     else if (k == "pdl") *value = h->pdl;
-    else if (k == "mpk_fused") *value = h->mpk_fused ? 1 : 0;
-    else if (k == "bandwidth") *value = h->bandwidth;
     else if (k == "uniform_diagonal") *value = h->dinv_uniform > 0.0 ? 1 : 0;
-    else if (k == "mpk_levels_per_pass") *value = h->mw_levels;
-    else if (k == "mpk_block_rows") *value = h->mw_block;
-    else if (k == "mpk_grid") *value = h->mw_grid;
-    else if (k == "mpk_lag") *value = h->mw_lag;
-    else if (k == "mpk_lag_dep") *value = h->mw_lag_dep;
     else if (k == "reordered") *value = h->reordered ? 1 : 0;
     else if (k == "cm_levels") *value = h->cm_levels;
     else if (k == "cm_components") *value = h->cm_comps;
@@ -1062,7 +936,6 @@ int sstep_cg_setup(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rowptr,
     if (int rc = setup_uniform_diagonal(h)) return rc;
     if (int rc = setup_spmv_variant(h)) return rc;
     if (int rc = setup_block_kernels(h)) return rc;
-    if (int rc = setup_mpk_wave(h)) return rc;
     if (int rc = setup_resident(h)) return rc;
     if (int rc = setup_workspaces(h)) return rc;
     if (int rc = setup_graph(h)) return rc;
@@ -1175,13 +1048,7 @@ int sstep_cg_profile_outer(sstep_cg_t* h, int reps, double* ms_host) {
         int e = 0;
         const int64_t n = h->n;
         for (int rep = 0; rep < reps; rep++) {
-            if (h->mpk_fused) {  // the whole MPK is one event pair; the other s - 1 pairs stay empty
-                CK(cudaEventRecord(evs[e++], sm));
-                CK(launch_mpk(h, sm, h->R, h->AR, h->st));
-                CK(cudaEventRecord(evs[e++], sm));
-                for (int j = 1; j < h->s; j++) { CK(cudaEventRecord(evs[e++], sm)); CK(cudaEventRecord(evs[e++], sm)); }
-            }
-            for (int j = 0; j < h->s && !h->mpk_fused; j++) {
+            for (int j = 0; j < h->s; j++) {
                 double* yjac = (j + 1 < h->s) ? h->R + (int64_t)(j + 1) * n : nullptr;
                 int mode = 0;
                 const double* xprev = nullptr;
@@ -1337,11 +1204,11 @@ int sstep_cg_solve_host(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rp
 
 // ---------------------------------------------------------------- measurement aid (measure.cuh)
 int sstep_cg_measure_bandwidth(sstep_cg_t* h, int variant, int64_t bytes, int passes, int reps, double* gbs_out) {
-    if (!h || !gbs_out || variant < 0 || variant > 3 || bytes < (1 << 20) || passes < 1 || reps < 1) return SSTEP_CG_ERR_ARG;
+    if (!h || !gbs_out || variant < 0 || variant > 5 || bytes < (1 << 20) || passes < 1 || reps < 1) return SSTEP_CG_ERR_ARG;
     if (h->in_solve) return fail(h, SSTEP_CG_ERR_STATE, "measure_bandwidth: a solve is in progress");
     CK(cudaSetDevice(h->device));
     cudaStream_t sm = h->stream;
-    bytes &= ~(int64_t)4095;
+    bytes &= ~(int64_t)8191;
     unsigned char *src = nullptr, *dst = nullptr;
     double* sink = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -1356,27 +1223,19 @@ int sstep_cg_measure_bandwidth(sstep_cg_t* h, int variant, int64_t bytes, int pa
         }
         CK(cudaEventCreate(&e0));
         CK(cudaEventCreate(&e1));
-        constexpr int CH1 = 4096, D1 = 2, CH3 = 2048, D3 = 4;
-        const size_t smem1 = (size_t)8 * D1 * CH1 + 8 * D1 * 8, smem3 = (size_t)8 * D3 * CH3 + 8 * D3 * 8;
-        int occ = 1, grid = h->num_sms;
+        int occ = 1;
         if (variant == 0) CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_ldg_kernel, 256, 0));
         if (variant == 2) CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_copy_kernel, 256, 0));
-        if (variant == 1) {
-            CK(cudaFuncSetAttribute(measure_read_bulk_kernel<D1, CH1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_bulk_kernel<D1, CH1>, 256, smem1));
-        }
-        if (variant == 3) {
-            CK(cudaFuncSetAttribute(measure_read_bulk_kernel<D3, CH3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3));
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, measure_read_bulk_kernel<D3, CH3>, 256, smem3));
-        }
-        grid = (occ < 1 ? 1 : occ) * h->num_sms;
+        const int grid = (occ < 1 ? 1 : occ) * h->num_sms;
         double best = 0.0, sum = 0.0;
         for (int rep = -1; rep < reps; rep++) {  // rep -1 = warm-up
             CK(cudaEventRecord(e0, sm));
             if (variant == 0) measure_read_ldg_kernel<<<grid, 256, 0, sm>>>((const double2*)src, bytes / 16, passes, sink);
-            else if (variant == 1) measure_read_bulk_kernel<D1, CH1><<<grid, 256, smem1, sm>>>(src, bytes / CH1, passes, sink);
-            else if (variant == 3) measure_read_bulk_kernel<D3, CH3><<<grid, 256, smem3, sm>>>(src, bytes / CH3, passes, sink);
-            else measure_copy_kernel<<<grid, 256, 0, sm>>>((const double2*)src, (double2*)dst, bytes / 16, passes);
+            else if (variant == 2) measure_copy_kernel<<<grid, 256, 0, sm>>>((const double2*)src, (double2*)dst, bytes / 16, passes);
+            else if (variant == 1) CK((launch_measure_bulk<2, 4096, 8>(h->num_sms, 3, sm, src, bytes, passes, sink)));   // 48 copies in flight per SM
+            else if (variant == 3) CK((launch_measure_bulk<4, 2048, 8>(h->num_sms, 3, sm, src, bytes, passes, sink)));   // 96
+            else if (variant == 4) CK((launch_measure_bulk<2, 8192, 4>(h->num_sms, 3, sm, src, bytes, passes, sink)));   // 24
+            else CK((launch_measure_bulk<2, 4096, 8>(h->num_sms, 2, sm, src, bytes, passes, sink)));                     // 32
             CK(cudaGetLastError());
             CK(cudaEventRecord(e1, sm));
             CK(cudaEventSynchronize(e1));

@@ -219,7 +219,7 @@ def test_x_may_alias_x0_and_peek_reports_history(oracle_mod, cg_mod, torch_mod):
 def test_measure_bandwidth_runs(cg_mod, torch_mod):
     """The measurement aid of bench.py's read-side peak: every variant returns a positive, plausible figure."""
     with cg_mod.SStepCG(0) as h:
-        for variant in (0, 1, 2, 3):
+        for variant in (0, 1, 2, 3, 4, 5):
             best, mean = h.measure_bandwidth(variant, 256 << 20, passes=1, reps=3)
             assert 100.0 < mean <= best < 20000.0, (variant, best, mean)
         best, _ = h.measure_bandwidth(0, 32 << 20, passes=20, reps=3)      # L2-resident sweep
