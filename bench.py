@@ -266,7 +266,7 @@ def run_ours(args):
             h.setup(rp, ci, va, s)
             torch.cuda.synchronize()
             t_setup = time.perf_counter() - t_setup
-            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_grid", "gram_grid", "update_grid", "reordered", "cm_levels", "pdl")}
+            info = {k: h.get_info(k) for k in ("lanes", "spmv_bulk", "spmv_cta", "spmv_grid", "gram_grid", "update_grid", "reordered", "cm_levels", "pdl")}
             info["setup_seconds"] = t_setup      # validation, dinv, (auto) Cuthill-McKee reordering, workspaces, graph capture
             if s == s0 and form == 0:
                 with ClockSampler(local) as clk:
@@ -531,7 +531,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)       # config 4: "fixed 200 outer iterations for timing"
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--s", type=int, default=4, help="block size of the headline value (paper uses s <= 5)")
+    ap.add_argument("--s", type=int, default=0, help="block size of the headline value (0 = the config's own: 2, 4, 4, 4, 8 for "
+                                                     "configs 1-5, 4 for the paper-shaped config 6; the paper uses s <= 5)")
     ap.add_argument("--grid", type=int, default=320, help="grid edge N of config 4 (N^3 unknowns)")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6],
                     help="BASELINE.json config (4 = the headline workload; the others fill BASELINE.md's table; 6 = the "
@@ -551,6 +552,8 @@ def main():
     args = ap.parse_args()
     args.extra = {kv.split("=", 1)[0]: int(kv.split("=", 1)[1]) for kv in args.opt}
     args.warmup = max(args.warmup, 3)
+    if args.s == 0:
+        args.s = {1: 2, 2: 4, 3: 4, 4: 4, 5: 8, 6: 4}[args.config]
 
     if args.impl == "reference":
         line = run_reference(args)
@@ -600,10 +603,12 @@ def main():
         "iteration_roofline": {"bound": "hbm", "achieved": p["achieved_gbs"], "peak": ctx["peak"], "unit": "GB/s",
                                "frac": p["frac_of_measured_peak"], "frac_of_nominal_8tbs": p["frac_of_nominal_8tbs"],
                                "algorithmic_bytes_per_outer": mb["total"]},
-        "roofline": {"bound": "hbm", "kernel": "spmv_bulk_kernel (Jacobi-fused CSR SpMV, s launches per outer iteration)"
-                     if p["spmv_bulk"] else "spmv_vec_kernel",
+        "roofline": {"bound": "hbm", "kernel": ("spmv_cta_kernel" if p.get("spmv_cta") else "spmv_bulk_kernel" if p["spmv_bulk"] else "spmv_vec_kernel")
+                     + " (Jacobi-fused CSR SpMV, s launches per outer iteration)",
                      "achieved": mb["spmv_per_launch"] / k_us / 1e3, "peak": ctx["peak"], "unit": "GB/s",
                      "frac": mb["spmv_per_launch"] / k_us / 1e3 / ctx["peak"], "peak_source": ctx["peak_src"],
+                     "read_peak": ctx["read_peak"]["read_peak_gbs"] if ctx["read_peak"] else None,
+                     "frac_of_read_peak": (mb["spmv_per_launch"] / k_us / 1e3 / ctx["read_peak"]["read_peak_gbs"]) if ctx["read_peak"] else None,
                      "algorithmic_bytes_per_launch": mb["spmv_per_launch"], "avg_launch_us": k_us,
                      "share_of_step": p["kernel_share_of_step"]["spmv"],
                      "traffic": ncu_traffic(args.config, s) if N == c_default_grid(args.config) else None,

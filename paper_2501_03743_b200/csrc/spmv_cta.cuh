@@ -1,5 +1,6 @@
-// spmv_cta.cuh -- step a1, thread-per-row matrices (mean row <= 8 entries: every 7-point config): the Jacobi-fused CSR
-// SpMV of the matrix-powers kernel (Alg. 4) with a CTA-wide producer / consumer TMA pipeline.
+// spmv_cta.cuh -- step a1 for stencil-like matrices (one lane per row: mean row <= 8 entries, every 7-point config; two lanes
+// per row: mean rows of 16-32 entries, the 27-point config): the Jacobi-fused CSR SpMV of the matrix-powers kernel
+// (Alg. 4) with a CTA-wide producer / consumer TMA pipeline.
 //
 // Why a second bulk-staged kernel (round 2).  The per-warp rings of spmv_bulk_kernel keep 24 warps x 2 slots x 2 arrays
 // = 96 bulk copies of ~1.3 KB in flight per SM.  Measured on this B200 with a pure streaming kernel (_work probe,
@@ -28,20 +29,21 @@
 // hence a valid index whose x cannot be non-finite unless the row's true result already is); `lo` must be a staged
 // index also for empty / dead rows.  Two phases, so that the caller can hand the stage back between them.  UNI: the diagonal is constant (every Poisson config), 1 / a_ii is a kernel argument
 // and the pick-up of a_ii from the row disappears; else diag returns the row's own diagonal entry.
+template <int U>
 struct StageRowFrag {
-    double v[8], xv[8];
+    double v[U], xv[U];
     double rem, diag;
 };
-// phase 1: fragment to registers, gathers issued (after it the stage may be handed back)
-template <bool UNI>
-__device__ __forceinline__ void stage_row_load(const double* sv, const int* sc, int lo, int hi, int row,
-                                               const double* __restrict__ x, StageRowFrag& f) {
-    constexpr int U = 8;
+// phase 1: fragment to registers, gathers issued (after it the stage may be handed back).  L lanes share a row: lane g of
+// the group takes the entries lo + g, lo + g + L, ...; U per lane live in registers, longer rows go through the remainder.
+template <bool UNI, int L, int U>
+__device__ __forceinline__ void stage_row_load(const double* sv, const int* sc, int lo, int hi, int row, int g,
+                                               const double* __restrict__ x, StageRowFrag<U>& f) {
     int c[U];
     f.diag = 0.0;
 #pragma unroll
     for (int u = 0; u < U; u++) {
-        const int kk = lo + u;
+        const int kk = lo + g + u * L;
         const bool ok = kk < hi;
         const int k2 = ok ? kk : lo;
         c[u] = sc[k2];
@@ -52,49 +54,50 @@ __device__ __forceinline__ void stage_row_load(const double* sv, const int* sc, 
 #pragma unroll
     for (int u = 0; u < U; u++) f.xv[u] = x[c[u]];
     double rem = 0.0;
-    for (int k0 = lo + U; k0 < hi; k0 += U) {  // rows longer than U entries: further batches
-        int cc[U];
-        double vv[U], xx[U];
+    for (int k0 = lo + g + U * L; k0 < hi; k0 += 8 * L) {  // rows longer than U L entries: further batches of 8 per lane
+        int cc[8];
+        double vv[8], xx[8];
 #pragma unroll
-        for (int u = 0; u < U; u++) {
-            const int kk = k0 + u;
+        for (int u = 0; u < 8; u++) {
+            const int kk = k0 + u * L;
             const bool ok = kk < hi;
             cc[u] = ok ? sc[kk] : -1;
             vv[u] = ok ? sv[kk] : 0.0;
             if (!UNI) { if (cc[u] == row) f.diag = vv[u]; }
         }
 #pragma unroll
-        for (int u = 0; u < U; u++) xx[u] = (cc[u] >= 0) ? x[cc[u]] : 0.0;
+        for (int u = 0; u < 8; u++) xx[u] = (cc[u] >= 0) ? x[cc[u]] : 0.0;
 #pragma unroll
-        for (int u = 0; u < U; u++) rem = fma(vv[u], xx[u], rem);
+        for (int u = 0; u < 8; u++) rem = fma(vv[u], xx[u], rem);
     }
     f.rem = rem;
 }
-// phase 2: the row sum (waits for the gathers)
-__device__ __forceinline__ double stage_row_sum(const StageRowFrag& f) {
+// phase 2: the lane's partial row sum (waits for the gathers); the caller adds the L lanes of a row with group_sum<L>
+template <int U>
+__device__ __forceinline__ double stage_row_sum(const StageRowFrag<U>& f) {
     double acc = 0.0;
 #pragma unroll
-    for (int u = 0; u < 8; u++) acc = fma(f.v[u], f.xv[u], acc);
+    for (int u = 0; u < U; u++) acc = fma(f.v[u], f.xv[u], acc);
     return acc + f.rem;
 }
 
-template <int D, int TR, int CAPT>
+template <int D, int TR, int CAPT, int L>
 struct SpmvCtaCfg {
-    static constexpr int NCW = TR / 32;                 // consumer warps
-    static constexpr int THREADS = TR + 32;             // + one producer warp
-    static constexpr size_t STAGE = (size_t)CAPT * 12;  // vals then cols of one stage
+    static constexpr int NCW = TR * L / 32;                  // consumer warps (a warp covers 32 / L rows)
+    static constexpr int THREADS = NCW * 32 + 32;            // + one producer warp
+    static constexpr size_t STAGE = (size_t)CAPT * 12;       // vals then cols of one stage
     static constexpr size_t SMEM = (size_t)D * STAGE + (size_t)D * 16 /* full, empty */ + (size_t)D * 8 /* a0 per stage */;
-    static_assert(CAPT % 4 == 0 && TR % 32 == 0, "stage sub-buffers must stay 16-byte aligned");
+    static_assert(CAPT % 4 == 0 && (TR * L) % 32 == 0, "stage sub-buffers must stay 16-byte aligned");
 };
 
-template <int D, int TR, int CAPT, bool MOM, int MINB, bool UNI>
-__global__ void __launch_bounds__(TR + 32, MINB)
+template <int D, int TR, int CAPT, bool MOM, int MINB, bool UNI, int L = 1, int U = 8>
+__global__ void __launch_bounds__(TR * L + 32, MINB)
 spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restrict__ ci, const double* __restrict__ va,
                 const double* __restrict__ x, double* __restrict__ y, double* __restrict__ yjac,
                 const double* __restrict__ xprev, int mode, const ScgState* __restrict__ st, int num_tiles,
                 double* __restrict__ mom_a, double* __restrict__ mom_b, double dinv_uniform) {
-    using Cfg = SpmvCtaCfg<D, TR, CAPT>;
-    constexpr int NCW = Cfg::NCW;
+    using Cfg = SpmvCtaCfg<D, TR, CAPT, L>;
+    constexpr int NCW = Cfg::NCW, RPW = 32 / L;  // rows per consumer warp
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* svals = reinterpret_cast<double*>(smem_raw);                                  // [D][CAPT]
     int* scols = reinterpret_cast<int*>(smem_raw + (size_t)D * CAPT * sizeof(double));    // [D][CAPT]
@@ -167,7 +170,7 @@ spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restric
     auto row_bounds = [&](int i, int& lo, int& hi) {
         lo = hi = 0;
         if (i < my_tiles) {
-            const int row = tile_row0(i) + warp * 32 + lane;
+            const int row = tile_row0(i) + warp * RPW + lane / L;
             if (row < n) { lo = rp[row]; hi = rp[row + 1]; }
         }
     };
@@ -179,7 +182,8 @@ spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restric
     for (int i = 0; i < tiles_eff; i++) {
         const int sl = i % D;
         const int lo = lo_n, hi = hi_n;
-        const int row = tile_row0(i) + warp * 32 + lane;
+        const int row = tile_row0(i) + warp * RPW + lane / L;
+        const int g = lane % L;
         row_bounds(i + 1, lo_n, hi_n);
         mbar_wait(&full[sl], (uint32_t)((i / D) & 1));
         if (!running) {  // stopped solver: hand the stage back, compute nothing
@@ -191,18 +195,19 @@ spmv_cta_kernel(int n, int nnz, const int* __restrict__ rp, const int* __restric
         const double* sv = svals + (size_t)sl * CAPT - a0;
         const int* sc = scols + (size_t)sl * CAPT - a0;
         const bool live = row < n;
-        StageRowFrag f;
-        stage_row_load<UNI>(sv, sc, live ? lo : a0, live ? hi : a0, row, x, f);
+        StageRowFrag<U> f;
+        stage_row_load<UNI, L, U>(sv, sc, live ? lo : a0, live ? hi : a0, row, g, x, f);
         double xrow = 0.0, xpv = 0.0;
-        if ((MOM || (jac && mode != 0)) && live) {
+        if ((MOM || (jac && mode != 0)) && live && g == 0) {
             xrow = x[row];
             if (mode == 2) xpv = xprev[row];
         }
         __syncwarp();  // every lane has read the stage
         if (lane == 0) mbar_arrive(&empty[sl]);
-        const double acc = stage_row_sum(f);
-        const double diag = f.diag;
-        if (live) {
+        const double acc = group_sum<L>(stage_row_sum<U>(f));
+        double diag = f.diag;
+        if (L > 1 && !UNI && jac) diag = group_sum<L>(diag);  // exactly one lane of the group holds a_ii, the others 0
+        if (live && g == 0) {
             y[row] = acc;
             if (MOM) ma = fma(xrow, acc, ma);
             if (jac) {

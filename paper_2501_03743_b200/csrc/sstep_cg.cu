@@ -42,6 +42,9 @@ constexpr size_t bulk_smem_for(int D, int cap, int wpc) { return (size_t)wpc * D
 // CTA-pipelined SpMV (spmv_cta.cuh), thread-per-row matrices: tiles of 256 rows, stage capacity 1800 entries (a 7-point
 // tile holds <= 1792; three stages x three CTAs = 194 KB of shared memory per SM, ~33 KB left for L1)
 constexpr int CTA_TR = 256, CTA_CAPT = 1800;
+// two lanes per row (mean rows of 16-32 entries: the 27-point config): tiles of 128 rows (8 consumer warps x 16 rows), stage
+// capacity 3472 entries (27 x 128 = 3456), 14 entries per lane in registers, two stages x two CTAs = 167 KB per SM
+constexpr int CTA2_TR = 128, CTA2_CAPT = 3472, CTA2_U = 14;
 
 }  // namespace
 
@@ -181,16 +184,24 @@ cta_fn_t cta_kernel_mu(int depth, int minb) {
 }
 cta_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
     const bool uni = h->dinv_uniform > 0.0;
+    if (h->lanes == 2) {
+        if (mom) return uni ? spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, true, 2, true, 2, CTA2_U> : spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, true, 2, false, 2, CTA2_U>;
+        return uni ? spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, false, 2, true, 2, CTA2_U> : spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, false, 2, false, 2, CTA2_U>;
+    }
     if (mom) return uni ? cta_kernel_mu<true, true>(h->cta_depth, h->cta_minb) : cta_kernel_mu<true, false>(h->cta_depth, h->cta_minb);
     return uni ? cta_kernel_mu<false, true>(h->cta_depth, h->cta_minb) : cta_kernel_mu<false, false>(h->cta_depth, h->cta_minb);
 }
-size_t cta_smem_for(int depth) { return (size_t)depth * CTA_CAPT * 12 + (size_t)depth * 24; }
+size_t cta_smem_for(const sstep_cg* h) {
+    const int depth = h->lanes == 2 ? 2 : h->cta_depth, capt = h->lanes == 2 ? CTA2_CAPT : CTA_CAPT;
+    return (size_t)depth * capt * 12 + (size_t)depth * 24;
+}
+int cta_per_sm(const sstep_cg* h) { return h->lanes == 2 ? 2 : h->cta_minb; }
 
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
-    if (L == 1 && h->cta) {
-        return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, CTA_TR + 32, cta_smem_for(h->cta_depth), sm, (int)h->n,
+    if ((L == 1 || L == 2) && h->cta) {
+        return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, CTA_TR + 32, cta_smem_for(h), sm, (int)h->n,
                         (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->cta_tiles, mom_a, mom_b, h->dinv_uniform);
     }
     if (h->bulk) {
@@ -219,8 +230,8 @@ template <int L>
 cudaError_t config_spmv_L(sstep_cg* h) {
     int occ = 0;
     cudaError_t e;
-    if (L == 1 && h->cta) {
-        const size_t smem = cta_smem_for(h->cta_depth);
+    if ((L == 1 || L == 2) && h->cta) {
+        const size_t smem = cta_smem_for(h);
         for (int mom = 0; mom < 2; mom++) {
             e = cudaFuncSetAttribute(cta_kernel_for(h, mom != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
@@ -228,7 +239,7 @@ cudaError_t config_spmv_L(sstep_cg* h) {
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cta_kernel_for(h, h->form != 0 || h->method == 1), CTA_TR + 32, smem);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
-        if (occ > h->cta_minb) occ = h->cta_minb;
+        if (occ > cta_per_sm(h)) occ = cta_per_sm(h);
         const int64_t cap = (int64_t)occ * h->num_sms;
         h->spmv_grid = (int)(h->cta_tiles < cap ? h->cta_tiles : cap);
         if (h->spmv_grid < 1) h->spmv_grid = 1;
@@ -657,23 +668,25 @@ int setup_spmv_variant(sstep_cg* h) {
     // thread-per-row matrices whose 256-row tiles fit a stage: the CTA-pipelined kernel (few large bulk copies in flight,
     // spmv_cta.cuh) replaces the per-warp rings -- auto, or forced with spmv_variant = 3 (2 keeps the per-warp rings)
     h->cta = false;
-    if (((h->spmv_variant == 0 && h->bulk && h->bulk_cap == BULK_CAP) || h->spmv_variant == 3) && L == 1 && aligned &&
+    if (h->spmv_variant == 3 && L == 4 && !h->lanes_opt) L = 2;  // (forced: the two-lane shape for mean rows of 16-32 entries)
+    if (((h->spmv_variant == 0 && h->bulk) || h->spmv_variant == 3) && (L == 1 || L == 2) && aligned &&
         n + 2 * CTA_TR < (int64_t(1) << 31)) {
-        const int64_t tiles = (n + CTA_TR - 1) / CTA_TR;
+        const int tr = (L == 2) ? CTA2_TR : CTA_TR, capt = (L == 2) ? CTA2_CAPT : CTA_CAPT;
+        const int64_t tiles = (n + tr - 1) / tr;
         CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
-        tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, CTA_TR, tiles, h->iscratch + 2);
+        tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, tr, tiles, h->iscratch + 2);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(hs + 2, h->iscratch + 2, sizeof(int), cudaMemcpyDeviceToHost, sm));
         CK(cudaStreamSynchronize(sm));
-        if (hs[2] + 3 <= CTA_CAPT) {
+        if (hs[2] + 3 <= capt) {
             h->cta = true;
             h->cta_tiles = (int)tiles;
         }
     }
     if (h->spmv_variant == 3 && !h->cta) {
         free_problem(h);
-        return fail(h, SSTEP_CG_ERR_ARG, "setup: CTA-pipelined SpMV forced but it needs one lane per row, 16 B aligned arrays and "
-                                         "256-row tiles of at most 1797 entries");
+        return fail(h, SSTEP_CG_ERR_ARG, "setup: CTA-pipelined SpMV forced but it needs one or two lanes per row, 16 B aligned arrays and "
+                                         "tiles (256 rows / 128 rows) of at most 1797 / 3469 entries");
     }
     h->lanes = L;
     return 0;

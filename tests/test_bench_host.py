@@ -92,3 +92,13 @@ def test_ncu_traffic_table_is_read():
     alg = bench.model_bytes(n, nnz, 4)["spmv_per_launch"]
     assert t is not None and 0.95 * alg < t < 1.15 * alg          # measured DRAM traffic within 15 % of the algorithmic bytes
     assert bench.ncu_traffic(4, 3) is None and bench.ncu_traffic(9, 4) is None
+
+
+def test_both_arms_print_the_same_workload_string():
+    """`vs_reference.same_config` was false only because the two arms spelt config.workload differently."""
+    import bench
+    n, nnz = 320 ** 3, 7 * 320 ** 3 - 6 * 320 ** 2
+    ours = bench.workload_string(4, 320, n, nnz, 4, "poisson7_320_sweep")
+    ref = bench.workload_string(4, 320, n, nnz, 4)
+    assert ours == ref and "320^3" in ours and f"nnz={nnz}" in ours and "s=4" in ours
+    assert "config 2" in bench.workload_string(2, 128, 128 ** 3, 1, 4, "poisson7_128_s4")

@@ -237,6 +237,24 @@ def test_rank_deficient_block_reports_breakdown(oracle_mod, cg_mod, torch_mod):
     assert abs(res["outer_iters"] - ref["iters"]) <= 1 and np.all(np.isfinite(x))
 
 
+def test_breakdown_contract_x_is_the_last_good_iterate(cg_mod, torch_mod):
+    """include/sstep_cg.h, SSTEP_CG_BREAKDOWN: a bad Cholesky pivot / non-finite Gram block is detected BEFORE the block
+    update, which is then skipped -- x comes back as the last good iterate.  Here the right-hand side is so large that
+    R_1 = D^-1 r overflows in the very first matrix-powers kernel: the first Gram block is non-finite, status 2 after
+    zero completed iterations, and x is exactly x0 (graph path and resident path)."""
+    c = gen.make_config(1, N=10)
+    t = lambda a: torch_mod.from_numpy(np.ascontiguousarray(a)).cuda()
+    x0 = np.random.default_rng(2).uniform(-1, 1, c["n"])
+    v = c["vals"] * 1e-170                                   # a_ii = 6e-170: dinv = 1.7e169; b ~ 1e150 -> R_1 overflows
+    b = np.sign(c["b"]) * 1e150
+    for resident in (1, 0):
+        with cg_mod.SStepCG(0, resident=resident) as h:
+            h.setup(t(c["rowptr"]), t(c["colidx"]), t(v), 2)
+            x, res = h.solve(t(b), x0=t(x0), rtol=1e-8, maxit=50)
+        assert res["status"] == 2 and res["status_name"] == "breakdown" and res["outer_iters"] == 0, res
+        assert np.array_equal(x.cpu().numpy(), x0)
+
+
 def test_invalid_arguments(cg_mod, torch_mod):
     rp, ci, v = gen.poisson1d(10)
     t = lambda a: dev(torch_mod, a)

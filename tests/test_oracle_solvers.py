@@ -247,3 +247,60 @@ def test_paper_514_iterations(oracle_mod):
     assert c["n"] == 250 ** 3 and c["nnz"] == 109_000_000
     res = oracle_mod.pfcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=1e-6, maxit=2000)
     assert res["status"] == 0 and res["iters"] == gold["pfcg_250cubed_1gpu"]
+
+
+# ------------------------------------------------------------------------------------------------ timing legs, fixtures
+def test_openmp_build_is_the_same_program_up_to_summation_order(oracle_mod):
+    """bench.py's all-core cpu_baseline leg: the same sstep_oracle.c built with -fopenmp.  Its row loops are the serial
+    ones (bitwise the same SpMV), its inner products are summed per thread (another order): after a few outer iterations
+    the iterate agrees with the serial build to rounding.  The in-loop clock excludes the start-up and reports a time."""
+    import sstep_inputs as gen
+    c = gen.make_config(2, N=20)
+    args = (c["rowptr"], c["colidx"], c["vals"], c["b"], 4, 5)
+    per1, start1, o1 = oracle_mod.sstep_timed(*args, omp=False)
+    per2, start2, o2 = oracle_mod.sstep_timed(*args, omp=True)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 4, rtol=0.0, maxit=5)
+    assert np.array_equal(o1["x"], ref["x"])                    # the time log does not touch the arithmetic
+    assert np.linalg.norm(o2["x"] - ref["x"]) <= 1e-10 * np.linalg.norm(ref["x"])
+    assert per1 > 0 and per2 > 0 and start1 >= 0 and start2 >= 0 and oracle_mod.omp_threads() >= 1
+    lib1, lib2 = oracle_mod.lib(False), oracle_mod.lib(True)
+    x = np.random.default_rng(3).uniform(-1, 1, c["n"])
+    y1 = np.empty(c["n"]); y2 = np.empty(c["n"])
+    import ctypes as C
+    for L, y in ((lib1, y1), (lib2, y2)):
+        L.orc_spmv(C.c_int64(c["n"]), c["rowptr"].ctypes.data_as(C.POINTER(C.c_int32)), c["colidx"].ctypes.data_as(C.POINTER(C.c_int32)),
+                   c["vals"].ctypes.data_as(C.POINTER(C.c_double)), x.ctypes.data_as(C.POINTER(C.c_double)), y.ctypes.data_as(C.POINTER(C.c_double)))
+    assert np.array_equal(y1, y2)
+
+
+def test_golden_fixtures_are_consistent_and_reproducible(oracle_mod, tmp_path):
+    """tests/golden/config*.txt (written by make_golden.py from the oracle alone): every fixture parses, is a converged
+    solve whose history ends below rtol at exactly `iters`, the paper's problem gives the paper's 514 at s = 1 and for
+    Alg. 1 and ceil(514 / s) for s = 2..5, and the writer reproduces itself on a small
+    grid (the format round-trips, the sample indices are the seeded ones)."""
+    import importlib.util, math, os
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden_cpu", os.path.join(gdir, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec); spec.loader.exec_module(mg)
+    paper = int([ln.split()[1] for ln in open(os.path.join(gdir, "paper_iterations.txt")) if ln.startswith("pfcg_250cubed_1gpu")][0])
+    for name, (cfg, s, basis, method) in mg.CASES.items():
+        g = mg.load(os.path.join(gdir, name + ".txt"))
+        assert g["config"] == cfg and g["s"] == s and g["basis"] == basis and g["method"] == method
+        assert g["status"] == 0 and g["iters"] == g["hist"].size and g["hist"][-1] < g["rtol"] <= g["hist"][-2]
+        assert g["xi"].size == mg.NS == g["nsample"] and np.array_equal(g["xi"], mg.sample_indices(g["n"]))
+        assert np.abs(g["xv"]).max() <= g["xmaxabs"] <= g["xnorm2"]
+        if cfg == 6:
+            assert g["iters"] == math.ceil(paper / s), (name, g["iters"])
+    assert mg.load(os.path.join(gdir, "config6_s1.txt"))["iters"] == paper == mg.load(os.path.join(gdir, "config6_pcg.txt"))["iters"]
+    # s-step iterates are CG iterates every s steps: the three config-4 solves end at the same point (PAPER.md:132-138)
+    g1, g2, g4 = (mg.load(os.path.join(gdir, f"config4_s{s}.txt")) for s in (1, 2, 4))
+    assert g2["iters"] == math.ceil(g1["iters"] / 2) and g4["iters"] == math.ceil(g1["iters"] / 4)
+    assert np.abs(g2["xv"] - g1["xv"]).max() <= 1e-9 and abs(g4["hist"][0] - g1["hist"][3]) <= 1e-9 * g1["hist"][3]
+    # writer -> reader on a grid the oracle finishes at once
+    mg.HERE = str(tmp_path)
+    out = mg.run_case("config4_s4", N=16)
+    g = mg.load(out)
+    import sstep_inputs as gen
+    c = gen.make_config(4, N=16)
+    ref = oracle_mod.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], 4, rtol=c["rtol"], maxit=c["maxit"], history=True)
+    assert g["iters"] == ref["iters"] and np.array_equal(g["hist"], ref["hist"]) and np.array_equal(g["xv"], ref["x"][g["xi"]])
