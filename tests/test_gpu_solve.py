@@ -295,6 +295,7 @@ def test_residual_replacement_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg,
     c = gen.make_config(cfg, N=N, s=s)
     rp, ci, v, b = c["rowptr"], c["colidx"], c["vals"], c["b"]
     K = 6
+    norm_inf_A = np.add.reduceat(np.abs(v), rp[:-1]).max()
     ref = oracle_mod.sstep(rp, ci, v, b, s, rtol=0.0, maxit=K, xhist_cap=K, history=True, replace_every=R)
     full = oracle_mod.sstep(rp, ci, v, b, s, rtol=c["rtol"], maxit=c["maxit"], replace_every=R)
     with cg_mod.SStepCG(0, replace_every=R) as h:
@@ -307,9 +308,12 @@ def test_residual_replacement_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg,
             x, res = h.solve_end()
             assert res["outer_iters"] == k and res["status"] == 1
             assert res["kernel_launches"] == 1 + k * (s + 2) + 2 * (k // R)
-            assert rel(x.cpu().numpy(), ref["xhist"][k - 1]) <= 1e-11
-            # (an iterate difference of 1e-11 moves a residual by up to ||A|| ||dx|| / ||b||: absolute floor 1e-13)
-            assert abs(res["relres"] - ref["hist"][k - 1]) <= 1e-9 * ref["hist"][k - 1] + 1e-13
+            xk = x.cpu().numpy()
+            assert rel(xk, ref["xhist"][k - 1]) <= 1e-11
+            # an iterate difference dx moves a residual norm by at most ||A dx|| <= ||A||_inf ||dx||_2 (A symmetric): that, not a
+            # fixed number, is the floor under the 1e-9 relative bar (27-point: ||A||_inf = 52)
+            floor = norm_inf_A * np.linalg.norm(xk - ref["xhist"][k - 1]) / np.linalg.norm(b) + 1e-14
+            assert abs(res["relres"] - ref["hist"][k - 1]) <= 1e-9 * ref["hist"][k - 1] + floor
             if k % R == 0:     # the reported residual is the true one (oracle's SpMV of the GPU's iterate)
                 true = np.linalg.norm(b - oracle_mod.spmv(rp, ci, v, x.cpu().numpy())) / np.linalg.norm(b)
                 # (b - A x cancels: its rounding error is ~1e-16 (||b|| + ||A|| ||x||), an absolute floor on the residual norm)
