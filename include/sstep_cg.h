@@ -232,6 +232,24 @@ int sstep_cg_test_small_solve_carried(sstep_cg_t *handle, const double *M, const
 int sstep_cg_test_update(sstep_cg_t *handle, double *R_cm, const double *AR_cm, double *P_il, double *AP_il,
                          double *x, double *r, const double *beta, const double *alpha, double *rho_out);
 
+/* ---- allocation-free entry point ----
+ * Step a2 (M = R^T AR, C = AP^T R, m = R^T r; Eq. 3-4; generalises Alg. 5) for callers that cannot
+ * call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  Needs only
+ * sstep_cg_create (no setup, no matrix).  Runs the production gram_kernel on a scratch array that is a STATIC part of
+ * the library image (364 544 bytes of every GPU that loads the library, until the process exits): the call itself
+ * performs no cudaMalloc / cudaFree and calls no allocating library routine -- three kernel launches on the handle's
+ * stream, nothing else; it returns without synchronising.
+ *   n >= 1 rows; 1 <= s <= 8 (LIMIT: the static scratch holds 2s^2+s <= 136 entries for at most 320 blocks; larger s is
+ *   rejected with SSTEP_CG_ERR_ARG and a text in sstep_cg_last_error).
+ *   R_cm, AR_cm: n x s column-major; AP_il: n x s interleaved; r: n   (device, read only)
+ *   M, C: s*s row-major; m: s                                          (device, caller-owned outputs)
+ * All calls on a device share the one array, which keeps the previous call's contents (the call clears what must start
+ * clean); calls that OVERLAP on the GPU -- two streams, two handles on the same device -- race on it: serialise them.
+ * Same summation scheme as the solver's Gram kernel (fixed order, reproducible run to run); the grid is capped at 320
+ * blocks, so the bits may differ from sstep_cg_test_gram's within the Gram tolerance. */
+int sstep_cg_gram_noalloc(sstep_cg_t *handle, int64_t n, int s, const double *R_cm, const double *AR_cm,
+                          const double *AP_il, const double *r, double *M, double *C, double *m);
+
 #ifdef __cplusplus
 }
 #endif

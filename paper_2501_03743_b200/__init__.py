@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
     "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update", "sstep_cg_test_read_state",
-    "sstep_cg_get_permutation",
+    "sstep_cg_get_permutation", "sstep_cg_gram_noalloc",
 ]
 
 
@@ -85,6 +85,7 @@ def load_library(build: bool = True):
     lib.sstep_cg_test_update.argtypes = [vp] + [vp] * 9
     lib.sstep_cg_test_read_state.argtypes = [vp, C.c_char_p, vp, i64]
     lib.sstep_cg_get_permutation.argtypes = [vp, vp]
+    lib.sstep_cg_gram_noalloc.argtypes = [vp, i64, i32] + [vp] * 7
     for name in EXPORTED_SYMBOLS:
         if name != "sstep_cg_last_error":
             getattr(lib, name).restype = C.c_int
@@ -308,6 +309,21 @@ class SStepCG:
         self._check(self._lib.sstep_cg_test_gram(self._h, self._ptr(R), self._ptr(AR), self._ptr(AP_il), self._ptr(r),
                                                  self._ptr(M), self._ptr(Cm), self._ptr(m)), "sstep_cg_test_gram")
         return M, Cm, m
+
+    def gram_noalloc(self, R, AR, AP_il, r, M, Cm, m):
+        """sstep_cg_gram_noalloc: a2 on the library's static scratch -- no allocation anywhere (the caller passes every
+        buffer, AP already in the interleaved (n, s) layout; outputs M, Cm (s, s) and m (s) are filled asynchronously on
+        the handle's stream).  Works after create alone; s <= 8."""
+        torch = _torch()
+        s, n = R.shape
+        ns = n * s
+        R, AR = self._dev(R, torch.float64, "R", ns), self._dev(AR, torch.float64, "AR", ns)
+        AP_il = self._dev(AP_il, torch.float64, "AP_il", ns)
+        r = self._dev(r, torch.float64, "r", n)
+        M, Cm = self._dev(M, torch.float64, "M", s * s), self._dev(Cm, torch.float64, "C", s * s)
+        m = self._dev(m, torch.float64, "m", s)
+        self._check(self._lib.sstep_cg_gram_noalloc(self._h, n, s, self._ptr(R), self._ptr(AR), self._ptr(AP_il), self._ptr(r),
+                                                    self._ptr(M), self._ptr(Cm), self._ptr(m)), "sstep_cg_gram_noalloc")
 
     def test_small_solve(self, M, Cm, m, Wprev):
         torch = _torch()

@@ -812,6 +812,76 @@ int setup_graph(sstep_cg* h) {
 
 }  // namespace
 
+// =============================================================================================== allocation-free Gram entry
+// sstep_cg_gram_noalloc (include/sstep_cg.h): the fused block inner products a2 for callers that cannot call cudaMalloc
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The production gram_kernel<S> needs
+// scratch memory -- an ScgState (ticket of the cross-block finish, the finished M, C, m) and the per-block partials
+// [2s^2+s][grid] -- which sstep_cg_setup takes from cudaMalloc.  Here the same kernel runs on a file-scope device array
+// of a fixed, modest size: NOALLOC_SMAX = 8 (2s^2+s <= 136 entries) x NOALLOC_MAX_BLOCKS = 320 blocks x 8 B = 348 160 B
+// + 16 KB for the state = 364 544 B, held by every GPU that loads the library until the process exits.
+// In host code the array's NAME is a host-side stand-in, not a device address (a kernel given it faults, or silently
+// uses host memory where the GPU can reach it): the address comes from cudaGetSymbolAddress, once per device, with that
+// device current, at set-up (sstep_cg_create), and is what the kernels receive.  Every call shares the array, which keeps
+// the previous call's contents: the reset kernel clears what must start clean (status, ticket); calls that overlap on the
+// GPU (two streams, two handles on one device) race on it.
+namespace {
+
+constexpr int NOALLOC_SMAX = 8;
+constexpr int NOALLOC_MAX_BLOCKS = 320;
+constexpr size_t NOALLOC_STATE_BYTES = 16384;
+constexpr size_t NOALLOC_SCRATCH_BYTES =
+    NOALLOC_STATE_BYTES + sizeof(double) * (size_t)NOALLOC_MAX_BLOCKS * (2 * NOALLOC_SMAX * NOALLOC_SMAX + NOALLOC_SMAX);
+static_assert(sizeof(ScgState) <= NOALLOC_STATE_BYTES, "the state must fit its share of the static scratch");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned char* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};  // device address of g_noalloc_scratch per device (set at create)
+
+// set-up, once per device, with that device current: the DEVICE address of the static array
+cudaError_t noalloc_setup_device(int device) {
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    if (g_noalloc_ptr[device]) return cudaSuccess;
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[device] = static_cast<unsigned char*>(ptr);
+    return cudaSuccess;
+}
+
+// clears what a call needs clean, whatever the previous call (or an aborted one) left behind
+__global__ void noalloc_reset_kernel(ScgState* st) {
+    st->status = SCG_RUNNING;  // gram_kernel leaves at once on any other status
+    st->ticket_gram = 0;
+}
+
+// results out of the static state into the caller's buffers (device code may name the array directly)
+__global__ void noalloc_output_kernel(int s, double* __restrict__ M, double* __restrict__ C, double* __restrict__ m) {
+    const ScgState* st = reinterpret_cast<const ScgState*>(g_noalloc_scratch);
+    for (int e = threadIdx.x; e < s * s; e += blockDim.x) { M[e] = st->M[e]; C[e] = st->C[e]; }
+    if ((int)threadIdx.x < s) m[threadIdx.x] = st->m[threadIdx.x];
+}
+
+template <int S>
+cudaError_t noalloc_gram_S(int num_sms, cudaStream_t sm, int64_t n, const double* R, const double* AR, const double* AP,
+                           const double* r, unsigned char* scratch) {
+    using Cfg = GramCfg<S>;
+    int occ = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_kernel<S>, Cfg::NW * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    int64_t grid = (n + Cfg::RG * 32 - 1) / (Cfg::RG * 32);
+    if (grid > (int64_t)occ * num_sms) grid = (int64_t)occ * num_sms;
+    if (grid > NOALLOC_MAX_BLOCKS) grid = NOALLOC_MAX_BLOCKS;  // partials [2s^2+s][grid] must fit the static array
+    ScgState* st = reinterpret_cast<ScgState*>(scratch);
+    double* partials = reinterpret_cast<double*>(scratch + NOALLOC_STATE_BYTES);
+    noalloc_reset_kernel<<<1, 1, 0, sm>>>(st);
+    gram_kernel<S><<<(unsigned)grid, Cfg::NW * 32, 0, sm>>>(n, R, AR, AP, r, partials, st, /*do_solve=*/0);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
 // =============================================================================================== C ABI
 extern "C" {
 
@@ -829,6 +899,7 @@ int sstep_cg_create(sstep_cg_t** handle, int device, void* cuda_stream) {
     h->stream = (cudaStream_t)cuda_stream;
     h->num_sms = prop.multiProcessorCount;
     bool ok = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && noalloc_setup_device(device) == cudaSuccess;  // device address of the static scratch of sstep_cg_gram_noalloc
     ok = ok && cudaMalloc(&h->st, sizeof(ScgState)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->st_test, sizeof(ScgState)) == cudaSuccess;
     ok = ok && cudaMalloc(&h->iscratch, 4 * sizeof(int)) == cudaSuccess;
@@ -1416,6 +1487,34 @@ int sstep_cg_test_update(sstep_cg_t* h, double* R, const double* AR, double* P, 
     CK(launch_update(h, h->stream, false, R, AR, P, AP, x, r, beta, alpha, h->st_test, rho_out));
     CK(cudaStreamSynchronize(h->stream));
     return 0;
+}
+
+int sstep_cg_gram_noalloc(sstep_cg_t* h, int64_t n, int s, const double* R, const double* AR, const double* AP,
+                          const double* r, double* M, double* C, double* m) {
+    if (!h || !R || !AR || !AP || !r || !M || !C || !m) return SSTEP_CG_ERR_ARG;
+    if (s < 1 || s > NOALLOC_SMAX)
+        return fail(h, SSTEP_CG_ERR_ARG, "gram_noalloc: block size s must be 1..8 (the static scratch holds 2s^2+s <= 136 entries per "
+                                         "block; use sstep_cg_setup + the solver, or sstep_cg_test_gram, for larger s)");
+    if (n < 1 || n >= (int64_t(1) << 40)) return fail(h, SSTEP_CG_ERR_ARG, "gram_noalloc: need 1 <= n < 2^40 rows");
+    unsigned char* scratch = (h->device < NOALLOC_MAX_DEVICES) ? g_noalloc_ptr[h->device] : nullptr;
+    if (!scratch) return fail(h, SSTEP_CG_ERR_STATE, "gram_noalloc: the static scratch of this device was not set up (sstep_cg_create does it)");
+    cudaStream_t sm = h->stream;
+    cudaError_t e = cudaSuccess;
+    switch (s) {
+        case 1: e = noalloc_gram_S<1>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 2: e = noalloc_gram_S<2>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 3: e = noalloc_gram_S<3>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 4: e = noalloc_gram_S<4>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 5: e = noalloc_gram_S<5>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 6: e = noalloc_gram_S<6>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        case 7: e = noalloc_gram_S<7>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+        default: e = noalloc_gram_S<8>(h->num_sms, sm, n, R, AR, AP, r, scratch); break;
+    }
+    if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("gram_noalloc: ") + cudaGetErrorString(e));
+    noalloc_output_kernel<<<1, 64, 0, sm>>>(s, M, C, m);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, SSTEP_CG_ERR_CUDA, std::string("gram_noalloc: ") + cudaGetErrorString(e));
+    return 0;  // asynchronous on the handle's stream, like every kernel launch
 }
 
 }  // extern "C"
