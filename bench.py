@@ -363,7 +363,9 @@ def run_ours(args):
             resident = dict(s=s0, us_per_outer=1e3 * agg["ms_per_step"], launches=launches, grid=h.get_info("resident_grid"),
                             rows_per_cta=h.get_info("resident_rows_per_block"), smem_bytes=h.get_info("resident_smem_bytes"),
                             gdof_iter_per_s=world * n * s0 / (1e3 * agg["ms_per_step"] * 1e-6) / 1e9, relres_at_end=res["relres"],
-                            note="whole loop in one cooperative launch per restart (csrc/resident.cuh); s + 1 grid barriers per outer iteration")
+                            sync=("tagged-word exchange between the CTAs, no grid barrier" if h.get_info("resident_sync") == 0
+                                  else "s + 1 grid barriers per outer iteration"),
+                            note="whole loop in one cooperative launch per restart (csrc/resident.cuh)")
     return dict(world=world, rank=rank, local=local, c=c, n=n, nnz=nnz, N=N, sweep=sweep, moment=moment, primary=primary, clocks=clocks,
                 resident=resident, pcg=pcg, sustained=sustained, read_peak=read_peak,
                 peak=peak, peak_src=peak_src, t_gen=t_gen, dev=(rp, ci, va, b))

@@ -94,6 +94,10 @@ struct sstep_cg {
     int cm_levels = 0, cm_comps = 0, far_permille = 0;
     // resident (cooperative, whole loop in one launch) path for problems that fit shared memory
     bool resident = false;
+    int resident_sync = 0;               // 0 = flag-in-data exchange between the CTAs (default) | 1 = grid barriers (round 1)
+    ulonglong2 *llR = nullptr, *llPart = nullptr, *llTot = nullptr;  // tagged exchange buffers of the resident kernel
+    size_t llR_bytes = 0, llPart_bytes = 0;  // (llTot has the size of llPart)
+    unsigned int ll_tag = 0;             // tags below or equal to this value have been used
     int res_grid = 0, res_rpb = 0, res_nzcap = 0, res_threads = 0;
     size_t res_smem = 0;
     cudaGraph_t graph = nullptr;
@@ -397,20 +401,25 @@ cudaError_t launch_update(sstep_cg* h, cudaStream_t sm, bool configure, double* 
 }
 
 // resident path (resident.cuh): op 0 = set the shared-memory attribute and report the occupancy, op 1 = cooperative launch
-template <int S>
-cudaError_t resident_S(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
+template <int S, bool LL>
+cudaError_t resident_SL(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
     if (op == 0) {
-        cudaError_t e = cudaFuncSetAttribute(resident_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->res_smem);
+        cudaError_t e = cudaFuncSetAttribute(resident_kernel<S, LL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->res_smem);
         if (e != cudaSuccess) return e;
-        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_out, resident_kernel<S>, h->res_threads, h->res_smem);
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_out, resident_kernel<S, LL>, h->res_threads, h->res_smem);
     }
     ResidentParams p;
     p.n = (int)h->n; p.rpb = h->res_rpb; p.nzcap = h->res_nzcap; p.kmax = kmax; p.basis = h->basis;
     p.rp = h->rp; p.ci = h->ci; p.va = h->va; p.dinv = h->dinv;
     p.Rg = h->R; p.ARg = h->AR; p.P = h->P; p.AP = h->AP; p.x = h->x; p.r = h->r;
     p.partials = h->partials; p.st = h->st;
+    p.llR = h->llR; p.llPart = h->llPart; p.llTot = h->llTot; p.tag0 = h->ll_tag;
     void* args[] = {&p};
-    return cudaLaunchCooperativeKernel((const void*)resident_kernel<S>, dim3(h->res_grid), dim3(h->res_threads), args, h->res_smem, sm);
+    return cudaLaunchCooperativeKernel((const void*)resident_kernel<S, LL>, dim3(h->res_grid), dim3(h->res_threads), args, h->res_smem, sm);
+}
+template <int S>
+cudaError_t resident_S(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
+    return h->resident_sync == 0 ? resident_SL<S, true>(h, sm, op, kmax, occ_out) : resident_SL<S, false>(h, sm, op, kmax, occ_out);
 }
 
 cudaError_t resident_op(sstep_cg* h, cudaStream_t sm, int op, int kmax, int* occ_out) {
@@ -483,6 +492,10 @@ void free_problem(sstep_cg* h) {
         if (*b) cudaFree(*b);
         *b = nullptr;
     }
+    if (h->llR) cudaFree(h->llR);
+    if (h->llPart) cudaFree(h->llPart);
+    if (h->llTot) cudaFree(h->llTot);
+    h->llR = h->llPart = h->llTot = nullptr;
     double** dbufs[] = {&h->own_pva, &h->bperm, &h->x0perm};
     for (double** b : dbufs) {
         if (*b) cudaFree(*b);
@@ -774,6 +787,17 @@ int setup_workspaces(sstep_cg* h) {
     if (np < 2 * (size_t)h->pcg_grid) np = 2 * (size_t)h->pcg_grid;
     if (np < (size_t)h->res_grid * (2 * s * s + s + 1)) np = (size_t)h->res_grid * (2 * s * s + s + 1);
     CK(cudaMalloc(&h->partials, sizeof(double) * np));
+    if (h->resident && h->resident_sync == 0) {  // tagged exchange buffers (resident.cuh, ll_*): all tags start at 0 = "nothing yet"
+        h->llR_bytes = sizeof(ulonglong2) * (size_t)n * s;
+        h->llPart_bytes = sizeof(ulonglong2) * 2 * (size_t)(2 * s * s + s + 1) * h->res_grid;
+        CK(cudaMalloc(&h->llR, h->llR_bytes));
+        CK(cudaMalloc(&h->llPart, h->llPart_bytes));
+        CK(cudaMalloc(&h->llTot, h->llPart_bytes));
+        CK(cudaMemsetAsync(h->llR, 0, h->llR_bytes, sm));
+        CK(cudaMemsetAsync(h->llPart, 0, h->llPart_bytes, sm));
+        CK(cudaMemsetAsync(h->llTot, 0, h->llPart_bytes, sm));
+        h->ll_tag = 0;
+    }
     CK(cudaMalloc(&h->mom, sizeof(double) * 2 * s * (size_t)h->spmv_grid));
     CK(cudaMemsetAsync(h->mom, 0, sizeof(double) * 2 * s * (size_t)h->spmv_grid, sm));
     CK(cudaMemsetAsync(h->R, 0, blk, sm));
@@ -949,6 +973,7 @@ int sstep_cg_set_option(sstep_cg_t* h, const char* key, int64_t value) {
     else if (k == "block_variant" && value >= 0 && value <= 2) h->block_variant = (int)value;
     else if (k == "form" && (value == 0 || value == 1)) h->form = (int)value;
     else if (k == "resident" && value >= 0 && value <= 2) h->resident_opt = (int)value;
+    else if (k == "resident_sync" && (value == 0 || value == 1)) h->resident_sync = (int)value;
     else if (k == "reorder" && value >= 0 && value <= 2) h->reorder_opt = (int)value;
     else if (k == "replace_every" && value >= 0 && value <= 1000000) h->replace_every = (int)value;
     else if (k == "method" && (value == 0 || value == 1)) h->method = (int)value;
@@ -991,6 +1016,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "far_permille") *value = h->far_permille;
     else if (k == "resident") *value = h->resident ? 1 : 0;
     else if (k == "resident_grid") *value = h->res_grid;
+    else if (k == "resident_sync") *value = h->resident_sync;
     else if (k == "resident_rows_per_block") *value = h->res_rpb;
     else if (k == "resident_smem_bytes") *value = (int64_t)h->res_smem;
     else return fail(h, SSTEP_CG_ERR_ARG, "unknown info key: " + k);
@@ -1072,8 +1098,19 @@ int sstep_cg_iterate(sstep_cg_t* h, int k_outer) {
         const int64_t kcap = (int64_t(1) << 31) / ((int64_t)h->res_grid * (h->s + 1)) - 1;
         for (int64_t done = 0; done < k_outer;) {
             const int k = (int)((k_outer - done < kcap) ? k_outer - done : kcap);
-            CK(cudaMemsetAsync(&h->st->grid_bar, 0, 33 * sizeof(unsigned int), h->stream));
+            if (h->resident_sync == 0) {
+                // tags of this launch: ll_tag + 1 .. ll_tag + k + 1; never reused -- before they could wrap, start over from zeroed buffers
+                if ((uint64_t)h->ll_tag + (uint64_t)k + 2 >= (uint64_t(1) << 31)) {
+                    CK(cudaMemsetAsync(h->llR, 0, h->llR_bytes, h->stream));
+                    CK(cudaMemsetAsync(h->llPart, 0, h->llPart_bytes, h->stream));
+                    CK(cudaMemsetAsync(h->llTot, 0, h->llPart_bytes, h->stream));
+                    h->ll_tag = 0;
+                }
+            } else {
+                CK(cudaMemsetAsync(&h->st->grid_bar, 0, 33 * sizeof(unsigned int), h->stream));
+            }
             CK(resident_op(h, h->stream, 1, k, nullptr));
+            if (h->resident_sync == 0) h->ll_tag += (unsigned int)k + 2u;
             h->launches++;
             h->graph_launches++;
             done += k;

@@ -184,6 +184,31 @@ def test_resident_and_graph_paths_agree(cg_mod, torch_mod):
     assert np.array_equal(x.cpu().numpy(), out[2][0])
 
 
+@pytest.mark.parametrize("cfg,N,s", [(1, 32, 2), (1, 24, 1), (2, 36, 4), (4, 30, 3)])
+def test_resident_exchange_modes_agree_bitwise(cg_mod, torch_mod, cfg, N, s):
+    """resident_sync = 0 (default: tagged-word exchange between the CTAs, no grid barrier, stop test one matrix-powers kernel
+    late) and resident_sync = 1 (round 1's grid barriers) run the same arithmetic in the same order: same iteration count,
+    same x bit for bit, for a converged solve and for a fixed number of iterations in several launches."""
+    c = gen.make_config(cfg, N=N, s=s)
+    out = {}
+    for sync in (0, 1):
+        with cg_mod.SStepCG(0, resident=2, resident_sync=sync) as h:
+            h.setup(dev(torch_mod, c["rowptr"]), dev(torch_mod, c["colidx"]), dev(torch_mod, c["vals"]), s)
+            assert h.get_info("resident") == 1 and h.get_info("resident_sync") == sync
+            b = dev(torch_mod, c["b"])
+            x, res = h.solve(b, rtol=c["rtol"], maxit=c["maxit"])
+            h.solve_begin(b, None, 0.0)
+            for k in (1, 2, 3):              # 6 iterations in three launches: state and tags carry over
+                h.iterate(k)
+            x6, res6 = h.solve_end()
+            out[sync] = (x.cpu().numpy(), res, x6.cpu().numpy(), res6)
+    assert out[0][1]["status"] == 0 == out[1][1]["status"]
+    assert out[0][1]["outer_iters"] == out[1][1]["outer_iters"] and out[0][1]["relres"] == out[1][1]["relres"]
+    assert np.array_equal(out[0][0], out[1][0])
+    assert out[0][3]["outer_iters"] == 6 == out[1][3]["outer_iters"] and out[0][3]["relres"] == out[1][3]["relres"]
+    assert np.array_equal(out[0][2], out[1][2])
+
+
 def test_resident_auto_selection_and_limits(cg_mod, torch_mod):
     t = lambda a: dev(torch_mod, a)
     rp, ci, v = gen.poisson7(32)
