@@ -112,6 +112,41 @@ __device__ __forceinline__ void warp_sum_arrays(const double* p, int64_t stride,
     }
 }
 
+// Sums over the 32 lanes of K values per lane at once, by recursive halving: in the step with lane offset OFF a lane keeps
+// one half of its values and hands the other half to its partner, so the values per lane halve while the lanes per sum
+// double -- ceil(K/2) + ceil(K/4) + ... shuffles (37 for K = 36) instead of 5 K (180) for K separate butterfly sums.  On
+// return v[t], t < nvalid (<= warp_reduce_many_count(K)), holds the complete sum of entry `base + t`; every entry is held by
+// exactly one lane of the warp (halves that are empty padding are tracked by nvalid); the summation order depends only on K.
+__host__ __device__ constexpr int warp_reduce_many_count(int k) {
+    for (int step = 0; step < 5; step++) k = (k + 1) / 2;
+    return k;
+}
+template <int KC, int OFF, int K>
+__device__ __forceinline__ void warp_reduce_many_step(double (&v)[K], int lane, int& base, int& nvalid) {
+    if constexpr (OFF >= 1) {
+        constexpr int H = (KC + 1) / 2;
+        const bool up = (lane & OFF) != 0;
+#pragma unroll
+        for (int i = 0; i < H; i++) {
+            const double lo = v[i];
+            const double hi = (i + H < KC) ? v[i + H] : 0.0;
+            const double send = up ? lo : hi;
+            const double keep = up ? hi : lo;
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+        }
+        if (up) { base += H; nvalid = nvalid > H ? nvalid - H : 0; }  // the upper half: slots [H, KC) of the old numbering
+        else nvalid = nvalid < H ? nvalid : H;
+        warp_reduce_many_step<H, OFF / 2, K>(v, lane, base, nvalid);
+    }
+}
+template <int K>
+__device__ __forceinline__ int warp_reduce_many(double (&v)[K], int lane, int& nvalid) {
+    int base = 0;
+    nvalid = K;
+    warp_reduce_many_step<K, 16, K>(v, lane, base, nvalid);
+    return base;
+}
+
 template <int L>
 __device__ __forceinline__ double group_sum(double v) {
 #pragma unroll

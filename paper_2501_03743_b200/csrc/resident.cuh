@@ -337,16 +337,20 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
                     accm[g] = fma(Rsel, rv, accm[g]);
                 }
             }
+            {  // all sums of the warp in one recursive-halving reduction (common.cuh)
+                double v[NACC];
 #pragma unroll
-            for (int g = 0; g < G; g++) {
+                for (int g = 0; g < G; g++) {
 #pragma unroll
-                for (int i = 0; i < S; i++) {
-                    const double a = warp_sum(accM[i][g]);
-                    const double b = warp_sum(accC[g][i]);
-                    if (lane == 0) { red[warp][i * G + g] = a; red[warp][S * G + g * S + i] = b; }
+                    for (int i = 0; i < S; i++) { v[i * G + g] = accM[i][g]; v[S * G + g * S + i] = accC[g][i]; }
+                    v[2 * S * G + g] = accm[g];
                 }
-                const double cc = warp_sum(accm[g]);
-                if (lane == 0) red[warp][2 * S * G + g] = cc;
+                int nv;
+                const int base = warp_reduce_many<NACC>(v, lane, nv);
+                constexpr int KF = warp_reduce_many_count(NACC);
+#pragma unroll
+                for (int t = 0; t < KF; t++)
+                    if (t < nv) red[warp][base + t] = v[t];
             }
             __syncthreads();
             for (int a = tid; a < NACC; a += bd) {
