@@ -356,6 +356,11 @@ cudaError_t update_SM(sstep_cg* h, cudaStream_t sm, bool configure, double* R, c
         return launch_k(h, update_tma_kernel<S, MOM>, h->update_grid, TC::THREADS, TC::SMEM, sm, h->n, R, AR, P, AP, x, r, h->dinv,
                         beta, alpha, h->partials, st, rho_out, (h->n + TC::T - 1) / TC::T);
     }
+    if constexpr (S == 1) {  // two rows per thread, 128-bit accesses (update.cuh); the grid of update_kernel<1> covers it
+        if (aligned16(R) && aligned16(AR) && aligned16(P) && aligned16(AP) && aligned16(x) && aligned16(r) && aligned16(h->dinv))
+            return launch_k(h, update1_kernel<MOM>, h->update_grid_reg, 256, 0, sm, h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
+                            h->partials, st, rho_out, h->dinv_uniform);
+    }
     return launch_k(h, update_kernel<S, MOM>, h->update_grid_reg, 256, 0, sm, h->n, R, AR, P, AP, x, r, h->dinv, beta, alpha,
                     h->partials, st, rho_out, h->dinv_uniform);
 }

@@ -169,6 +169,59 @@ update_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, 
     update_block_finish<MOM>(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
 }
 
+// ---- s = 1: every stream (R, AR, P, AP, x, r) is a plain contiguous vector, and six 8-byte loads per thread leave too few
+// bytes in flight (update_kernel<1> ran at 0.89 of the copy peak on 320^3).  Two consecutive rows per thread, 128-bit
+// loads and stores: twice the bytes in flight at the same occupancy.  Per row the same operations in the same order as
+// update_half<1>; needs 16-byte aligned buffers (the caller falls back to update_kernel<1> otherwise).
+template <bool MOM>
+__global__ void __launch_bounds__(256, 4)
+update1_kernel(int64_t n, double* __restrict__ R, const double* __restrict__ AR, double* __restrict__ P,
+               double* __restrict__ AP, double* __restrict__ x, double* __restrict__ r, const double* __restrict__ dinv,
+               const double* __restrict__ beta_g, const double* __restrict__ alpha_g, double* __restrict__ partials,
+               ScgState* __restrict__ st, double* __restrict__ rho_out, double dinv_uniform) {
+    pdl_wait();
+    pdl_launch();
+    if (st->status != SCG_RUNNING) return;
+    const double beta = beta_g[0], alpha = alpha_g[0];
+    double rho = 0.0, mu0 = 0.0;
+    const int64_t npairs = n >> 1;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    auto one_row = [&](double Rv, double ARv, double Pv, double APv, double xv, double rv, double di, double& Pn, double& APn,
+                       double& xn, double& rn, double& r1) {
+        Pn = fma(Pv, beta, Rv);          // P <- R + P beta
+        xn = fma(Pn, alpha, xv);         // x += P alpha        (update_half: acc = fma(sign * p, alpha, acc), sign = +1)
+        APn = fma(APv, beta, ARv);       // AP <- AR + AP beta
+        rn = fma(-1.0 * APn, alpha, rv); // r -= AP alpha       (sign = -1)
+        r1 = di * rn;
+        rho = fma(rn, rn, rho);
+        if (MOM) mu0 = fma(r1, rn, mu0);
+    };
+    for (int64_t pr = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; pr < npairs; pr += stride) {
+        const int64_t row = 2 * pr;
+        const double2 Rv = *reinterpret_cast<const double2*>(R + row), ARv = *reinterpret_cast<const double2*>(AR + row);
+        const double2 Pv = *reinterpret_cast<const double2*>(P + row), APv = *reinterpret_cast<const double2*>(AP + row);
+        const double2 xv = *reinterpret_cast<const double2*>(x + row), rv = *reinterpret_cast<const double2*>(r + row);
+        double2 di = make_double2(dinv_uniform, dinv_uniform);
+        if (!(dinv_uniform > 0.0)) di = *reinterpret_cast<const double2*>(dinv + row);
+        double2 Pn, APn, xn, rn, r1;
+        one_row(Rv.x, ARv.x, Pv.x, APv.x, xv.x, rv.x, di.x, Pn.x, APn.x, xn.x, rn.x, r1.x);
+        one_row(Rv.y, ARv.y, Pv.y, APv.y, xv.y, rv.y, di.y, Pn.y, APn.y, xn.y, rn.y, r1.y);
+        *reinterpret_cast<double2*>(P + row) = Pn;
+        *reinterpret_cast<double2*>(AP + row) = APn;
+        *reinterpret_cast<double2*>(x + row) = xn;
+        *reinterpret_cast<double2*>(r + row) = rn;
+        *reinterpret_cast<double2*>(R + row) = r1;  // R(:,1) of the next outer iteration
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {  // odd n: the last row
+        const int64_t row = n - 1;
+        const double di = (dinv_uniform > 0.0) ? dinv_uniform : dinv[row];
+        double Pn, APn, xn, rn, r1;
+        one_row(R[row], AR[row], P[row], AP[row], x[row], r[row], di, Pn, APn, xn, rn, r1);
+        P[row] = Pn; AP[row] = APn; x[row] = xn; r[row] = rn; R[row] = r1;
+    }
+    update_block_finish<MOM>(rho, mu0, (int)(blockDim.x >> 5), partials, st, rho_out);
+}
+
 // ---- residual replacement (option "replace_every", reading A22): r <- b - A x with y = A x from the
 // production SpMV, R(:,1) <- D^-1 r, rho = ||r||^2 and the stop test taken again on the replaced residual.  P, AP stay.
 __global__ void __launch_bounds__(256)
