@@ -45,6 +45,9 @@ constexpr int CTA_TR = 256, CTA_CAPT = 1800;
 // two lanes per row (mean rows of 16-32 entries: the 27-point config): tiles of 128 rows (8 consumer warps x 16 rows), stage
 // capacity 3472 entries (27 x 128 = 3456), 14 entries per lane in registers, two stages x two CTAs = 167 KB per SM
 constexpr int CTA2_TR = 128, CTA2_CAPT = 3472, CTA2_U = 14;
+// ... and, when no moment partials ride on the SpMV (Gram form), tiles of 96 rows on THREE CTAs per SM: 208.5 instead of 213 us
+// per launch on 27-point 160^3 (the instantiation with the moment epilogue spills at that register budget: 314 us)
+constexpr int CTA2B_TR = 96, CTA2B_CAPT = 2608;
 
 }  // namespace
 
@@ -79,6 +82,7 @@ struct sstep_cg {
     int bulk_cap = 256, bulk_wpc = 8;
     bool cta = false;             // thread-per-row matrices: CTA-pipelined SpMV (spmv_cta.cuh) instead of the per-warp rings
     int cta_depth = 2, cta_minb = 3, cta_tiles = 0;
+    bool cta2_small = false;      // two lanes per row: the 96-row / three-CTA shape (Gram-form handles)
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0, pcg_grid = 0;
     bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
@@ -189,6 +193,8 @@ cta_fn_t cta_kernel_mu(int depth, int minb) {
 cta_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
     const bool uni = h->dinv_uniform > 0.0;
     if (h->lanes == 2) {
+        if (h->cta2_small)  // Gram-form handles only: never launched with moment partials
+            return uni ? spmv_cta_kernel<2, CTA2B_TR, CTA2B_CAPT, false, 3, true, 2, CTA2_U> : spmv_cta_kernel<2, CTA2B_TR, CTA2B_CAPT, false, 3, false, 2, CTA2_U>;
         if (mom) return uni ? spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, true, 2, true, 2, CTA2_U> : spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, true, 2, false, 2, CTA2_U>;
         return uni ? spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, false, 2, true, 2, CTA2_U> : spmv_cta_kernel<2, CTA2_TR, CTA2_CAPT, false, 2, false, 2, CTA2_U>;
     }
@@ -196,16 +202,17 @@ cta_fn_t cta_kernel_for(const sstep_cg* h, bool mom) {
     return uni ? cta_kernel_mu<false, true>(h->cta_depth, h->cta_minb) : cta_kernel_mu<false, false>(h->cta_depth, h->cta_minb);
 }
 size_t cta_smem_for(const sstep_cg* h) {
-    const int depth = h->lanes == 2 ? 2 : h->cta_depth, capt = h->lanes == 2 ? CTA2_CAPT : CTA_CAPT;
+    const int depth = h->lanes == 2 ? 2 : h->cta_depth, capt = h->lanes == 2 ? (h->cta2_small ? CTA2B_CAPT : CTA2_CAPT) : CTA_CAPT;
     return (size_t)depth * capt * 12 + (size_t)depth * 24;
 }
-int cta_per_sm(const sstep_cg* h) { return h->lanes == 2 ? 2 : h->cta_minb; }
+int cta_threads(const sstep_cg* h) { return (h->lanes == 2 ? 2 * (h->cta2_small ? CTA2B_TR : CTA2_TR) : CTA_TR) + 32; }  // consumer warps + the producer warp
+int cta_per_sm(const sstep_cg* h) { return h->lanes == 2 ? (h->cta2_small ? 3 : 2) : h->cta_minb; }
 
 template <int L>
 cudaError_t launch_spmv_L(sstep_cg* h, cudaStream_t sm, const double* x, double* y, double* yjac, const double* xprev,
                           int mode, const ScgState* st, double* mom_a, double* mom_b) {
     if ((L == 1 || L == 2) && h->cta) {
-        return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, CTA_TR + 32, cta_smem_for(h), sm, (int)h->n,
+        return launch_k(h, cta_kernel_for(h, mom_a != nullptr), h->spmv_grid, cta_threads(h), cta_smem_for(h), sm, (int)h->n,
                         (int)h->nnz, h->rp, h->ci, h->va, x, y, yjac, xprev, mode, st, h->cta_tiles, mom_a, mom_b, h->dinv_uniform);
     }
     if (h->bulk) {
@@ -240,7 +247,7 @@ cudaError_t config_spmv_L(sstep_cg* h) {
             e = cudaFuncSetAttribute(cta_kernel_for(h, mom != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
         }
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cta_kernel_for(h, h->form != 0 || h->method == 1), CTA_TR + 32, smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, cta_kernel_for(h, h->form != 0 || h->method == 1), cta_threads(h), smem);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
         if (occ > cta_per_sm(h)) occ = cta_per_sm(h);
@@ -689,7 +696,8 @@ int setup_spmv_variant(sstep_cg* h) {
     if (h->spmv_variant == 3 && L == 4 && !h->lanes_opt) L = 2;  // (forced: the two-lane shape for mean rows of 16-32 entries)
     if (((h->spmv_variant == 0 && h->bulk) || h->spmv_variant == 3) && (L == 1 || L == 2) && aligned &&
         n + 2 * CTA_TR < (int64_t(1) << 31)) {
-        const int tr = (L == 2) ? CTA2_TR : CTA_TR, capt = (L == 2) ? CTA2_CAPT : CTA_CAPT;
+        h->cta2_small = (L == 2) && h->form == 0 && h->method == 0;
+        const int tr = (L == 2) ? (h->cta2_small ? CTA2B_TR : CTA2_TR) : CTA_TR, capt = (L == 2) ? (h->cta2_small ? CTA2B_CAPT : CTA2_CAPT) : CTA_CAPT;
         const int64_t tiles = (n + tr - 1) / tr;
         CK(cudaMemsetAsync(h->iscratch + 2, 0, sizeof(int), sm));
         tile_nnz_max_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, sm>>>(n, rowptr, tr, tiles, h->iscratch + 2);
@@ -704,7 +712,7 @@ int setup_spmv_variant(sstep_cg* h) {
     if (h->spmv_variant == 3 && !h->cta) {
         free_problem(h);
         return fail(h, SSTEP_CG_ERR_ARG, "setup: CTA-pipelined SpMV forced but it needs one or two lanes per row, 16 B aligned arrays and "
-                                         "tiles (256 rows / 128 rows) of at most 1797 / 3469 entries");
+                                         "tiles (256 rows / 128 or 96 rows) of at most 1797 / 3469 or 2605 entries");
     }
     h->lanes = L;
     return 0;
