@@ -87,8 +87,16 @@ __device__ __forceinline__ double ll_value(const ulonglong2& w) {
 // Polled words must not be SHARED between many CTAs: when all 148 CTAs polled the same ~200 lines of partials (a flat
 // all-gather) the L2 slices holding them saturated and the stores being waited for queued behind the polls -- 5-7 us per
 // all-gather, 9 us after the last store; a __nanosleep back-off made it 11 us.  Hence the reduce-scatter + private inboxes below.
+// Every wait is bounded: a word that has not arrived after LL_SPIN_LIMIT poll rounds (tens of seconds; a healthy exchange
+// takes microseconds) can only mean a broken protocol or a lost peer -- the kernel traps (the launch returns an error)
+// instead of hanging the device.
+constexpr unsigned int LL_SPIN_LIMIT = 1u << 26;
 __device__ __forceinline__ void ll_wait(ulonglong2& w, const ulonglong2* p, unsigned int tag) {
-    while (!ll_ready(w, tag)) w = ll_peek(p);
+    unsigned int spins = 0;
+    while (!ll_ready(w, tag)) {
+        if (++spins > LL_SPIN_LIMIT) __trap();
+        w = ll_peek(p);
+    }
 }
 // the value published at p under `tag` (waits until it has arrived)
 __device__ __forceinline__ double ll_load(const ulonglong2* p, unsigned int tag) {
@@ -100,12 +108,13 @@ __device__ __forceinline__ double ll_load(const ulonglong2* p, unsigned int tag)
 // two SMs of an idle B200) per round -- waiting for them one after the other costs a round trip per stale word.
 template <int K, class PtrOf>
 __device__ __forceinline__ void ll_wait_all(ulonglong2 (&w)[K], PtrOf ptr_of, unsigned int valid, unsigned int tag) {
-    for (;;) {
+    for (unsigned int spins = 0;; spins++) {
         unsigned int pend = 0;
 #pragma unroll
         for (int k = 0; k < K; k++)
             if (((valid >> k) & 1u) && !ll_ready(w[k], tag)) pend |= 1u << k;
         if (!pend) return;
+        if (spins > LL_SPIN_LIMIT) __trap();
 #pragma unroll
         for (int k = 0; k < K; k++)
             if ((pend >> k) & 1u) w[k] = ll_peek(ptr_of(k));
