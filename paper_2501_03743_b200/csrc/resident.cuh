@@ -86,7 +86,8 @@ __device__ __forceinline__ double ll_value(const ulonglong2& w) {
 }
 // Polled words must not be SHARED between many CTAs: when all 148 CTAs polled the same ~200 lines of partials (a flat
 // all-gather) the L2 slices holding them saturated and the stores being waited for queued behind the polls -- 5-7 us per
-// all-gather, 9 us after the last store; a __nanosleep back-off made it 11 us.  Hence the reduce-scatter + private inboxes below.
+// all-gather, 9 us after the last store; a __nanosleep back-off made it 11 us; with the batched re-polling of ll_wait_all
+// still 3.5 us against 2.45 us for the two hops of the reduce-scatter + private inboxes below.
 // Every wait is bounded: a word that has not arrived after LL_SPIN_LIMIT poll rounds (tens of seconds; a healthy exchange
 // takes microseconds) can only mean a broken protocol or a lost peer -- the kernel traps (the launch returns an error)
 // instead of hanging the device.
