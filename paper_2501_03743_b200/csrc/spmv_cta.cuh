@@ -3,8 +3,8 @@
 // (Alg. 4) with a CTA-wide producer / consumer TMA pipeline.
 //
 // Why a second bulk-staged kernel (round 2).  The per-warp rings of spmv_bulk_kernel keep 24 warps x 2 slots x 2 arrays
-// = 96 bulk copies of ~1.3 KB in flight per SM.  Measured on this B200 with a pure streaming kernel (_work probe,
-// numbers in DESIGN.md section 6): the 1-D bulk-copy path of an SM runs at full speed only up to ~32 copies in flight --
+// = 96 bulk copies of ~1.3 KB in flight per SM.  Measured on this B200 with a pure streaming kernel
+// (sstep_cg_measure_bandwidth variants 2-5, measure.cuh; numbers in DESIGN.md section 6): the 1-D bulk-copy path of an SM runs at full speed only up to ~32 copies in flight --
 // 16-32 copies of >= 4 KB stream 7.2-7.3 TB/s from HBM and 18 TB/s from L2, 48 copies 6.0-7.5 TB/s from either, 96
 // copies 3.6 TB/s.  So the bytes in flight must come from FEW, LARGE copies: here one producer warp per CTA streams
 // tiles of TR = 256 rows (colidx + vals of the whole tile = two copies of ~14 KB + ~7 KB) into a ring of D stages, and
