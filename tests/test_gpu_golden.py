@@ -123,6 +123,25 @@ def test_config4_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod, s
     check_against_golden(oracle_mod, cg_mod, torch_mod, f"config4_s{s}", x_tol=1e-8, hist_tol=1e-6 if s <= 3 else 1e-4)
 
 
+@pytest.mark.parametrize("name,opts,resident", [
+    ("config1_s2", {}, 1),                    # 32^3: the default is the resident single-launch path (tagged-word exchange)
+    ("config1_s2", {"resident": 1}, 0),       # ... and the graph path on the same fixture
+    ("config2_s4", {}, 0),                    # 128^3, one lane per row (spmv_cta_kernel L = 1)
+    ("config3_s4", {}, 0),                    # 160^3 27-point, two lanes per row (spmv_cta_kernel L = 2)
+])
+def test_configs_1_to_3_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod, name, opts, resident):
+    """BASELINE.json configs[0..2] at full size and their own s, rtol: the small case the resident path serves, the
+    128^3 case and the 27-point case whose SpMV is round 2's two-lane CTA pipeline -- whole solves, like config 4."""
+    g = load_golden(name)
+    c, rp, ci, va, b = config_on_device(torch_mod, g["config"])
+    with cg_mod.SStepCG(0, **opts) as h:      # which path runs: asserted, not assumed
+        h.setup(rp, ci, va, g["s"])
+        assert h.get_info("resident") == resident
+        if not resident:
+            assert h.get_info("spmv_cta") == 1 and h.get_info("lanes") == (2 if g["config"] == 3 else 1)
+    check_against_golden(oracle_mod, cg_mod, torch_mod, name, x_tol=1e-8, hist_tol=1e-6 if g["s"] <= 3 else 1e-4, **opts)
+
+
 def test_config5_chebyshev_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod):
     """Config 5 (256^3 variable coefficients, permuted rows -> auto-reordered, s = 8) with the Chebyshev basis."""
     check_against_golden(oracle_mod, cg_mod, torch_mod, "config5_s8_cheb", x_tol=1e-8, hist_tol=1e-6)
