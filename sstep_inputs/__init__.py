@@ -22,7 +22,7 @@ import numpy as np
 
 __all__ = [
     "poisson7", "poisson7_box", "apply_poisson7_box", "poisson27", "varcoef7", "varcoef_cells", "apply_poisson7", "apply_poisson27",
-    "apply_varcoef7", "symmetric_permute", "random_spd_csr", "poisson1d",
+    "apply_varcoef7", "symmetric_permute", "random_spd_csr", "random_structure_spd_csr", "STRUCTURE_KINDS", "poisson1d",
     "make_config", "CONFIG_NAMES",
 ]
 
@@ -255,6 +255,87 @@ def random_spd_csr(n: int, density: float, seed: int, max_row: int | None = None
     np.cumsum(nzmask.sum(axis=1), out=rowptr[1:])
     cols = np.nonzero(nzmask)[1].astype(np.int32)
     return rowptr.astype(np.int32), cols, A[nzmask], A
+
+
+STRUCTURE_KINDS = ("banded", "uniform_lengths", "stencil_long_rows", "box7", "box27", "power_law", "near_diagonal")
+
+
+def random_structure_spd_csr(seed: int, kind: str | None = None, n: int | None = None):
+    """Seeded symmetric, strictly diagonally dominant (hence spd) CSR matrix whose SPARSITY STRUCTURE is drawn from one of
+    STRUCTURE_KINDS -- row lengths from 1 to thousands, banded or scattered columns, sizes from 1 row to 3e5 rows that are
+    deliberately not multiples of any tile -- for the random-structure parity tests (every SpMV kernel, lane count and
+    tile shape must either take the matrix and be right, or refuse it at setup).  Off-diagonal values U[-1, 0) (an
+    M-matrix pattern like the paper's discretisations), diagonal = factor * sum|off-diagonal| + U[0.01, 1], constant over
+    the rows with probability 0.3 where the structure allows it.  Returns (rowptr, colidx, vals, kind, n)."""
+    rng = np.random.default_rng([seed, 0x5717])
+    if kind is None:
+        kind = STRUCTURE_KINDS[int(rng.integers(0, len(STRUCTURE_KINDS)))]
+    if n is None:
+        n = int(rng.choice([1, 2, 31, 32, 33, 255, 256, 257, 1000, 4097, 20000, 65537, 150001, 300000]))
+
+    def band(offsets):
+        offsets = np.array(sorted({int(o) for o in offsets if 0 < abs(int(o)) < n}), dtype=np.int64)
+        rr = [np.arange(max(0, -o), min(n, n - o), dtype=np.int64) for o in offsets]
+        return (np.concatenate(rr) if rr else np.zeros(0, np.int64),
+                np.concatenate([r + o for r, o in zip(rr, offsets)]) if rr else np.zeros(0, np.int64))
+
+    if kind == "banded":
+        rows, cols = band(rng.integers(-min(n - 1, 3000), min(n - 1, 3000) + 1, int(rng.integers(0, 20))) if n > 1 else [])
+    elif kind == "uniform_lengths":
+        lens = rng.integers(0, int(rng.integers(1, 33)) + 1, n)
+        rows = np.repeat(np.arange(n, dtype=np.int64), lens)
+        cols = rng.integers(0, n, rows.size)
+    elif kind == "stencil_long_rows":
+        rows, cols = band([-1, 1])
+        for i in rng.choice(n, size=min(n, 5), replace=False):
+            js = rng.choice(n, size=int(rng.integers(1, min(n, 6000) + 1)), replace=False)
+            rows = np.concatenate([rows, np.full(js.size, i, np.int64)]); cols = np.concatenate([cols, js])
+    elif kind in ("box7", "box27"):
+        lo, hi = (1, 40) if kind == "box7" else (2, 30)
+        nx, ny, nz = (int(rng.integers(lo, hi)) for _ in range(3))
+        n = nx * ny * nz
+        i = np.arange(n, dtype=np.int64)
+        x, y, z = i % nx, (i // nx) % ny, i // (nx * ny)
+        rr, cc = [], []
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx in (-1, 0, 1):
+                    if (dx, dy, dz) == (0, 0, 0) or (kind == "box7" and abs(dx) + abs(dy) + abs(dz) != 1):
+                        continue
+                    ok = (x + dx >= 0) & (x + dx < nx) & (y + dy >= 0) & (y + dy < ny) & (z + dz >= 0) & (z + dz < nz)
+                    rr.append(i[ok]); cc.append(i[ok] + dx + nx * (dy + ny * dz))
+        rows = np.concatenate(rr) if rr else np.zeros(0, np.int64)
+        cols = np.concatenate(cc) if cc else np.zeros(0, np.int64)
+    elif kind == "power_law":
+        lens = np.minimum(np.minimum(n, 2000), np.maximum(0, (rng.pareto(1.2, n) * 2).astype(np.int64)))
+        rows = np.repeat(np.arange(n, dtype=np.int64), lens)
+        cols = rng.integers(0, n, rows.size)
+    elif kind == "near_diagonal":
+        k = n // 2 if n > 3 else 0
+        rows, cols = rng.integers(0, n, k), rng.integers(0, n, k)
+    else:
+        raise ValueError(f"unknown structure kind {kind!r}")
+    # symmetric pattern without the diagonal, one entry per (row, col)
+    keep = rows != cols
+    rows, cols = rows[keep], cols[keep]
+    key = np.unique(np.concatenate([rows * n + cols, cols * n + rows]))
+    rows, cols = key // n, key % n
+    upper = rows < cols
+    w = np.zeros(key.size)
+    w[upper] = rng.uniform(-1.0, 0.0, int(upper.sum())) - 1e-3
+    # the mirrored entry takes the same value: (c, r) sits at the position of key c * n + r
+    w[np.searchsorted(key, cols[upper] * n + rows[upper])] = w[upper]
+    offsum = np.bincount(rows, weights=np.abs(w), minlength=n)
+    diag = offsum * rng.uniform(1.0, 1.3) + rng.uniform(0.01, 1.0, n)
+    if rng.random() < 0.3:
+        diag = np.full(n, float(diag.max()))
+    allr = np.concatenate([rows, np.arange(n, dtype=np.int64)])
+    allc = np.concatenate([cols, np.arange(n, dtype=np.int64)])
+    allv = np.concatenate([w, diag])
+    order = np.lexsort((allc, allr))
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(np.bincount(allr, minlength=n), out=rowptr[1:])
+    return rowptr.astype(np.int32), allc[order].astype(np.int32), allv[order], kind, n
 
 
 # --------------------------------------------------------------------------

@@ -98,6 +98,33 @@ def test_random_spd_is_spd_and_irregular():
     assert lens.max() >= 30 and lens.min() <= 10
 
 
+def test_random_structure_matrices_meet_the_csr_contract():
+    """random_structure_spd_csr: every structure kind gives a symmetric, strictly diagonally dominant matrix with the
+    diagonal present once and positive, columns ascending and unique in a row, seeded (same seed, same matrix); the
+    kinds differ in what they are for -- long rows, ragged boxes, rows of one entry."""
+    for k, kind in enumerate(gen.STRUCTURE_KINDS):
+        for n in (1, 2, 33, 700):
+            rp, ci, v, kind_out, n_out = gen.random_structure_spd_csr(40 + k, kind, n)
+            assert kind_out == kind and rp.size == n_out + 1 and rp[-1] == ci.size == v.size
+            assert rp.dtype == np.int32 and ci.dtype == np.int32 and v.dtype == np.float64
+            if kind not in ("box7", "box27"):
+                assert n_out == n
+            A = _dense(rp, ci, v)
+            assert np.array_equal(A, A.T)
+            d = np.diag(A)
+            assert np.all(d > 0) and np.all(d > np.abs(A).sum(axis=1) - d)
+            for i in range(n_out):
+                row = ci[rp[i]:rp[i + 1]]
+                assert np.all(np.diff(row) > 0) and np.count_nonzero(row == i) == 1
+            again = gen.random_structure_spd_csr(40 + k, kind, n)
+            assert np.array_equal(again[0], rp) and np.array_equal(again[1], ci) and np.array_equal(again[2], v)
+    lens = lambda kind: np.diff(gen.random_structure_spd_csr(3, kind, 5000)[0])
+    assert lens("stencil_long_rows").max() > 1000 and lens("power_law").max() > 200 and lens("near_diagonal").min() == 1
+    assert lens("box27").max() == 27 and lens("box7").max() == 7
+    kinds = {gen.random_structure_spd_csr(seed, n=50)[3] for seed in range(40)}
+    assert kinds == set(gen.STRUCTURE_KINDS)
+
+
 def test_configs_are_seeded_and_consistent():
     a = gen.make_config(1, N=6)
     b = gen.make_config(1, N=6)
