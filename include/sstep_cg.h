@@ -233,6 +233,11 @@ int sstep_cg_test_small_solve(sstep_cg_t *handle, const double *M, const double 
 int sstep_cg_test_small_solve_carried(sstep_cg_t *handle, const double *M, const double *C, const double *m,
                                       const double *Lprev, double *beta, double *alpha, double *W, double *Lout,
                                       int32_t *status_out);
+/* The division inside the register version of a3 (resident path, s <= 2; csrc/small_solve.cuh): the IEEE quotient a / b
+ * computed as "reciprocal of b prepared once, three operations per dividend".  q[i] must equal the correctly rounded
+ * a[i] / b[i] bit for bit for ANY operands (zeros, subnormals, infinities, NaN -> NaN).  a, b, q: n device doubles;
+ * needs sstep_cg_create only. */
+int sstep_cg_test_division(sstep_cg_t *handle, int64_t n, const double *a, const double *b, double *q);
 /* a4, in place: P, AP (interleaved), x, r updated; R_cm(:,1) <- D^-1 r_new; rho_out[0] = ||r_new||^2. */
 int sstep_cg_test_update(sstep_cg_t *handle, double *R_cm, const double *AR_cm, double *P_il, double *AP_il,
                          double *x, double *r, const double *beta, const double *alpha, double *rho_out);

@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "converged", 1: "maxit", 2: "breakdown"}
 EXPORTED_SYMBOLS = [
     "sstep_cg_create", "sstep_cg_setup", "sstep_cg_set_option", "sstep_cg_get_info", "sstep_cg_solve",
     "sstep_cg_solve_begin", "sstep_cg_iterate", "sstep_cg_solve_end", "sstep_cg_solve_peek", "sstep_cg_profile_outer",
-    "sstep_cg_measure_bandwidth", "sstep_cg_test_small_solve_carried", "sstep_cg_solve_host", "sstep_cg_destroy",
+    "sstep_cg_measure_bandwidth", "sstep_cg_test_small_solve_carried", "sstep_cg_test_division", "sstep_cg_solve_host", "sstep_cg_destroy",
     "sstep_cg_last_error", "sstep_cg_test_spmv", "sstep_cg_test_mpk", "sstep_cg_test_mpk_moments", "sstep_cg_test_sw",
     "sstep_cg_test_gram",
     "sstep_cg_test_small_solve", "sstep_cg_test_update", "sstep_cg_test_read_state",
@@ -72,6 +72,7 @@ def load_library(build: bool = True):
     lib.sstep_cg_profile_outer.argtypes = [vp, i32, C.POINTER(dbl)]
     lib.sstep_cg_measure_bandwidth.argtypes = [vp, i32, i64, i32, i32, C.POINTER(dbl)]
     lib.sstep_cg_test_small_solve_carried.argtypes = [vp] + [vp] * 9
+    lib.sstep_cg_test_division.argtypes = [vp, C.c_int64, vp, vp, vp]
     lib.sstep_cg_solve_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, dbl, i32, C.POINTER(_Result)]
     lib.sstep_cg_destroy.argtypes = [vp]
     lib.sstep_cg_last_error.argtypes = [vp]
@@ -353,6 +354,15 @@ class SStepCG:
                                                                 self._ptr(beta), self._ptr(alpha), self._ptr(W), self._ptr(L),
                                                                 self._ptr(st)), "sstep_cg_test_small_solve_carried")
         return int(st.item()), beta, alpha, W, L
+
+    def test_division(self, a, b):
+        """q = a / b elementwise by the prepared-divisor division of the register-resident solves (see sstep_cg.h)."""
+        torch = _torch()
+        n = a.numel()
+        a, b = self._dev(a, torch.float64, "a", n), self._dev(b, torch.float64, "b", n)
+        q = torch.empty(n, dtype=torch.float64, device=a.device)
+        self._check(self._lib.sstep_cg_test_division(self._h, n, self._ptr(a), self._ptr(b), self._ptr(q)), "sstep_cg_test_division")
+        return q
 
     def test_read_state(self, name: str):
         """One internal array of the current solve state (see sstep_cg.h): blocks come back as (s, n) tensors."""

@@ -75,6 +75,14 @@ __device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * 
     // a warp owns the entries warp, warp + nwarps, ...; up to three of them per pass, their loads in flight together
     // (KB = 1, 2 for s = 1, 2: no more registers than the streaming loop of those kernels needs)
     constexpr int KB = (NE <= 8) ? 1 : (NE <= 16) ? 2 : 3;
+    // the last warp also fetches the Cholesky factor of the previous outer iteration's W: loads issued before its share of
+    // the sums, so that their latency is not added to the chain sums -> barrier -> solves
+    constexpr int NLQ = (S * S + 31) / 32;
+    double lreg[NLQ];
+    if (warp == nwarps - 1) {
+#pragma unroll
+        for (int q = 0; q < NLQ; q++) lreg[q] = (lane + 32 * q < S * S) ? st->Lw[lane + 32 * q] : 0.0;
+    }
     for (int e = warp; e < NE; e += KB * nwarps) {
         double v[KB];
         const int kv = (NE - e + nwarps - 1) / nwarps;
@@ -85,8 +93,11 @@ __device__ __forceinline__ void gram_cross_block_finish(const double (*red)[2 * 
                 if (e + q * nwarps < NE) fin[e + q * nwarps] = v[q];
         }
     }
-    if (warp == nwarps - 1)
-        for (int e = lane; e < S * S; e += 32) ssm.L[e] = st->Lw[e];  // Cholesky factor of the previous outer iteration's W
+    if (warp == nwarps - 1) {
+#pragma unroll
+        for (int q = 0; q < NLQ; q++)
+            if (lane + 32 * q < S * S) ssm.L[lane + 32 * q] = lreg[q];
+    }
     __syncthreads();
     if (warp == 0) {
         for (int e = lane; e < S * S; e += 32) { st->M[e] = fin[e]; st->C[e] = fin[S * S + e]; }

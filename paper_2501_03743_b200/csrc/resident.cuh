@@ -252,6 +252,7 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
         if (tid == 0) s_rho_cta = 0.0;
     }
     __syncthreads();
+    if (S <= 2 && warp == 0) warp_prepare_divisors(S, ssm.L, ssm.Rd, lane);  // (for thread_small_solve below, which keeps them in step with ssm.L)
 
     // A thread owns the rows lr = tid, tid + bd, ... in every phase, so the per-row shared-memory entries need no
     // barrier between phases; barriers are only needed around the cross-thread reductions.
@@ -416,15 +417,18 @@ __global__ void __launch_bounds__(512, 1) resident_kernel(const ResidentParams p
             // (ssm.L carries the Cholesky factor of W from one outer iteration to the next: one factorisation each)
             int rc;
             if constexpr (S <= 2) {  // in registers, fully unrolled, same operations and roundings (small_solve.cuh)
-                double Lc[S * S], be[S * S], al[S], Wn[S * S];
+                double Lc[S * S], Rc[S], be[S * S], al[S], Wn[S * S];
 #pragma unroll
                 for (int e = 0; e < S * S; e++) Lc[e] = ssm.L[e];
-                rc = thread_small_solve<S>(fin, fin + S * S, fin + 2 * S * S, Lc, be, al, Wn);
+#pragma unroll
+                for (int i = 0; i < S; i++) Rc[i] = ssm.Rd[i];
+                rc = thread_small_solve<S>(fin, fin + S * S, fin + 2 * S * S, Lc, Rc, be, al, Wn);
+                __syncwarp();  // every lane has read ssm.L / ssm.Rd
                 if (lane == 0 && rc == 0) {
 #pragma unroll
                     for (int e = 0; e < S * S; e++) { sbeta[e] = be[e]; sW[e] = Wn[e]; ssm.L[e] = Lc[e]; }
 #pragma unroll
-                    for (int i = 0; i < S; i++) salpha[i] = al[i];
+                    for (int i = 0; i < S; i++) { salpha[i] = al[i]; ssm.Rd[i] = Rc[i]; }
                 }
             } else {
                 rc = warp_small_solve(S, fin, fin + S * S, fin + 2 * S * S, nullptr, sbeta, salpha, sW, ssm, lane, /*have_L=*/true);

@@ -1529,6 +1529,17 @@ int sstep_cg_test_small_solve_carried(sstep_cg_t* h, const double* M, const doub
     return 0;
 }
 
+int sstep_cg_test_division(sstep_cg_t* h, int64_t n, const double* a, const double* b, double* q) {
+    if (!h || n < 0 || (n > 0 && (!a || !b || !q))) return SSTEP_CG_ERR_ARG;
+    if (n == 0) return 0;
+    CK(cudaSetDevice(h->device));
+    const int blocks = (int)std::min<int64_t>((n + 255) / 256, (int64_t)h->num_sms * 8);
+    division_test_kernel<<<blocks, 256, 0, h->stream>>>(n, a, b, q);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
 int sstep_cg_test_update(sstep_cg_t* h, double* R, const double* AR, double* P, double* AP, double* x, double* r,
                          const double* beta, const double* alpha, double* rho_out) {
     if (!h || !R || !AR || !P || !AP || !x || !r || !beta || !alpha) return SSTEP_CG_ERR_ARG;
