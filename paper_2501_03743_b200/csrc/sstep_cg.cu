@@ -75,6 +75,7 @@ struct sstep_cg {
     int* iscratch = nullptr;      // [err, max_len, max_tile]
     // owned copies made by solve_host
     int *own_rp = nullptr, *own_ci = nullptr;
+    int64_t own_n = 0, own_nnz = 0;  // sizes the owned copies were allocated for (solve_host reuses them call to call)
     double *own_va = nullptr, *own_b = nullptr, *own_x = nullptr;
     // kernel configuration
     int lanes = 1;
@@ -526,6 +527,7 @@ void free_owned(sstep_cg* h) {
     if (h->own_x) cudaFree(h->own_x);
     h->own_rp = h->own_ci = nullptr;
     h->own_va = h->own_b = h->own_x = nullptr;
+    h->own_n = h->own_nnz = 0;
 }
 
 int kernels_per_outer(const sstep_cg* h) {
@@ -1316,12 +1318,16 @@ int sstep_cg_solve_host(sstep_cg_t* h, int64_t n, int64_t nnz, const int32_t* rp
     cudaStream_t sm = h->stream;
     CK(cudaStreamSynchronize(sm));
     free_problem(h);
-    free_owned(h);
-    CK(cudaMalloc(&h->own_rp, sizeof(int) * (n + 1)));
-    CK(cudaMalloc(&h->own_ci, sizeof(int) * nnz));
-    CK(cudaMalloc(&h->own_va, sizeof(double) * nnz));
-    CK(cudaMalloc(&h->own_b, sizeof(double) * n));
-    CK(cudaMalloc(&h->own_x, sizeof(double) * n));
+    if (!(h->own_x && h->own_n == n && h->own_nnz == nnz)) {  // a repeated call with the same sizes keeps its device copies' storage
+        free_owned(h);
+        CK(cudaMalloc(&h->own_rp, sizeof(int) * (n + 1)));
+        CK(cudaMalloc(&h->own_ci, sizeof(int) * nnz));
+        CK(cudaMalloc(&h->own_va, sizeof(double) * nnz));
+        CK(cudaMalloc(&h->own_b, sizeof(double) * n));
+        CK(cudaMalloc(&h->own_x, sizeof(double) * n));
+        h->own_n = n;
+        h->own_nnz = nnz;
+    }
     CK(cudaMemcpyAsync(h->own_rp, rp, sizeof(int) * (n + 1), cudaMemcpyHostToDevice, sm));
     CK(cudaMemcpyAsync(h->own_ci, ci, sizeof(int) * nnz, cudaMemcpyHostToDevice, sm));
     CK(cudaMemcpyAsync(h->own_va, va, sizeof(double) * nnz, cudaMemcpyHostToDevice, sm));

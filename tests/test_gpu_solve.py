@@ -288,6 +288,27 @@ def test_solve_host_end_to_end(oracle_mod, cg_mod, torch_mod):
     assert rel(x.numpy(), ref["x"]) <= 1e-8
 
 
+def test_solve_host_repeated_calls_on_one_handle(oracle_mod, cg_mod, torch_mod):
+    """sstep_cg_solve_host keeps the storage of its device copies for the next call when the sizes are the same (what a
+    serving loop and bench.py's e2e leg do): a second system of the SAME sizes but other values and another right-hand side,
+    then a system of other sizes, then the first again -- each against the oracle, nothing left over from the call before."""
+    th = lambda a: torch_mod.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    c1 = gen.make_config(1, N=16)
+    k = gen.varcoef_cells(16, 9)
+    rp2, ci2, v2 = gen.varcoef7(16, k)                              # same n and nnz as the 16^3 Poisson matrix, other values
+    assert rp2.size == c1["rowptr"].size and ci2.size == c1["colidx"].size
+    b2 = np.random.default_rng(12).uniform(-1, 1, rp2.size - 1)
+    c3 = gen.make_config(3, N=9)
+    systems = [(c1["rowptr"], c1["colidx"], c1["vals"], c1["b"], 2), (rp2, ci2, v2, b2, 3),
+               (c3["rowptr"], c3["colidx"], c3["vals"], c3["b"], 4), (c1["rowptr"], c1["colidx"], c1["vals"], c1["b"], 2)]
+    with cg_mod.SStepCG(0) as h:
+        for rp, ci, v, b, s in systems:
+            ref = oracle_mod.sstep(rp, ci, v, b, s, rtol=1e-8, maxit=500)
+            x, res = h.solve_host(th(rp), th(ci), th(v), th(b), s, rtol=1e-8, maxit=500)
+            assert ref["status"] == 0 and res["status"] == 0 and abs(res["outer_iters"] - ref["iters"]) <= 1
+            assert rel(x.numpy(), ref["x"]) <= 1e-8
+
+
 @pytest.mark.parametrize("cfg,N,s,R", [(2, 20, 3, 2), (1, 24, 2, 1), (5, 16, 4, 3), (3, 12, 4, 2)])
 def test_residual_replacement_matches_oracle(oracle_mod, cg_mod, torch_mod, cfg, N, s, R):
     """Option replace_every (reading A22) against the oracle's orc_sstep_rr: iterates, reported residuals
