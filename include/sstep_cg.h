@@ -164,7 +164,9 @@ int sstep_cg_solve_peek(sstep_cg_t *handle, sstep_cg_result *out);
 
 /* End-to-end convenience with HOST buffers: uploads CSR, b, x0 (NULL = zeros),
  * runs setup + solve on a private device copy, downloads x.  This is the call
- * bench.py's `e2e` number times. */
+ * bench.py's `e2e` number times.  The device copy belongs to the handle: its storage is
+ * kept for the next call with the same n and nnz (contents are uploaded afresh every call),
+ * replaced when the sizes change and released by sstep_cg_destroy. */
 int sstep_cg_solve_host(sstep_cg_t *handle, int64_t n, int64_t nnz, const int32_t *rowptr_host,
                         const int32_t *colidx_host, const double *vals_host, const double *b_host,
                         const double *x0_host, double *x_host, int s, double rtol, int maxit,
