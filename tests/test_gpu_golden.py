@@ -142,6 +142,30 @@ def test_configs_1_to_3_converged_solve_matches_golden(oracle_mod, cg_mod, torch
     check_against_golden(oracle_mod, cg_mod, torch_mod, name, x_tol=1e-8, hist_tol=1e-6 if g["s"] <= 3 else 1e-4, **opts)
 
 
+def test_config4_solve_host_matches_golden(oracle_mod, cg_mod, torch_mod):
+    """The call bench.py's `e2e` leg times -- ONE sstep_cg_solve_host with pinned HOST buffers: upload, setup, the whole
+    solve to rtol = 1e-8, download -- on the headline workload, against the same oracle-written fixture: count, status,
+    the 2048 sampled entries of x within 1e-8 of max|x|, ||x||_2; twice on one handle (the second call reuses the storage
+    of the first one's device copies)."""
+    g = load_golden("config4_s4")
+    c, *_ = config_on_device(torch_mod, 4)
+    pin = lambda a: torch_mod.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    rp, ci, va, b = pin(c["rowptr"]), pin(c["colidx"]), pin(c["vals"]), pin(c["b"])
+    x = torch_mod.empty(c["n"], dtype=torch_mod.float64).pin_memory()
+    with cg_mod.SStepCG(0) as h:
+        for call in range(2):
+            x.fill_(float("nan"))
+            _, res = h.solve_host(rp, ci, va, b, g["s"], rtol=g["rtol"], maxit=c["maxit"], x_out=x)
+            assert res["status"] == 0 and abs(res["outer_iters"] - g["iters"]) <= 1, (call, res)
+            xh = x.numpy()
+            if res["outer_iters"] == g["iters"]:
+                assert np.abs(xh[g["xi"]] - g["xv"]).max() <= 1e-8 * g["xmaxabs"], call
+                assert abs(np.linalg.norm(xh) - g["xnorm2"]) <= 1e-8 * g["xnorm2"]
+            else:      # one iteration more or less than the oracle: x differs by that step; the solution bar still holds
+                assert np.abs(xh[g["xi"]] - g["xv"]).max() <= 1e-6 * g["xmaxabs"], call
+            assert np.all(np.isfinite(xh))
+
+
 def test_config5_chebyshev_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod):
     """Config 5 (256^3 variable coefficients, permuted rows -> auto-reordered, s = 8) with the Chebyshev basis."""
     check_against_golden(oracle_mod, cg_mod, torch_mod, "config5_s8_cheb", x_tol=1e-8, hist_tol=1e-6)
