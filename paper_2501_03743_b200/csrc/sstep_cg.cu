@@ -85,7 +85,8 @@ struct sstep_cg {
     int cta_depth = 2, cta_minb = 3, cta_tiles = 0;
     bool cta2_small = false;      // two lanes per row: the 96-row / three-CTA shape (Gram-form handles)
     int spmv_grid = 0, gram_grid = 0, update_grid = 0, init_grid = 0, pcg_grid = 0;
-    bool staged = false;  // Gram / update through the TMA tile pipeline (s >= 5)
+    bool staged = false;       // update through the TMA tile pipeline (s >= 5)
+    bool staged_gram = false;  // Gram through the TMA tile pipeline (every s: see gram_tma.cuh)
     int gram_grid_reg = 0, update_grid_reg = 0;  // grids of the register kernels (used by hooks on misaligned buffers)
     int gram_tile = 0, gram_depth = 0, update_tile = 0, update_depth = 0;  // staged kernels: rows per tile, ring slots (0 = not staged)
     int64_t num_tiles = 0;
@@ -311,7 +312,7 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
         int64_t want = (h->n + Cfg::RG * 32 - 1) / (Cfg::RG * 32);
         int64_t cap = (int64_t)occ * h->num_sms;
         h->gram_grid_reg = h->gram_grid = (int)(want < cap ? want : cap);
-        if (h->staged) {
+        if (h->staged_gram) {
             e = cudaFuncSetAttribute(gram_tma_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC::SMEM);
             if (e != cudaSuccess) return e;
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, gram_tma_kernel<S>, TC::THREADS, TC::SMEM);
@@ -322,11 +323,11 @@ cudaError_t gram_S(sstep_cg* h, cudaStream_t sm, bool configure, const double* R
             h->gram_grid = (int)(want < cap ? want : cap);
             if (h->gram_grid < h->gram_grid_reg) h->gram_grid_reg = h->gram_grid;  // partials are sized by gram_grid
         }
-        h->gram_tile = h->staged ? TC::T : 0;
-        h->gram_depth = h->staged ? TC::D : 0;
+        h->gram_tile = h->staged_gram ? TC::T : 0;
+        h->gram_depth = h->staged_gram ? TC::D : 0;
         return cudaSuccess;
     }
-    if (h->staged && aligned16(R) && aligned16(AR) && aligned16(AP) && aligned16(r)) {
+    if (h->staged_gram && aligned16(R) && aligned16(AR) && aligned16(AP) && aligned16(r)) {
         return launch_k(h, gram_tma_kernel<S>, h->gram_grid, TC::THREADS, TC::SMEM, sm, h->n, R, AR, AP, r, h->partials, st, do_solve,
                         (h->n + TC::T - 1) / TC::T);
     }
@@ -726,6 +727,10 @@ int setup_block_kernels(sstep_cg* h) {
     const int s = h->s;
     cudaStream_t sm = h->stream;
     h->staged = (h->block_variant == 2) || (h->block_variant == 0 && s >= 5);
+    // Gram: staged for every s >= 5; for s = 2..4 on systems of >= 3 M rows, where its few large copies in flight read at 0.955
+    // of the read bandwidth against 0.924 for the register kernel (below that the one-CTA-per-SM ramp costs more than it gains;
+    // s = 1 gains nothing)
+    h->staged_gram = (h->block_variant == 2) || (h->block_variant == 0 && (s >= 5 || (s >= 2 && n >= 3000000)));
     CK(config_spmv(h));
     CK(launch_gram(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, 0));
     CK(launch_update(h, sm, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr));
@@ -1007,6 +1012,7 @@ int sstep_cg_get_info(sstep_cg_t* h, const char* key, int64_t* value) {
     else if (k == "spmv_depth") *value = h->spmv_depth;
     else if (k == "bulk_cap") *value = h->bulk ? h->bulk_cap : 0;
     else if (k == "block_staged") *value = h->staged ? 1 : 0;
+    else if (k == "gram_staged") *value = h->staged_gram ? 1 : 0;
     else if (k == "form") *value = h->form;
     else if (k == "gram_grid") *value = h->gram_grid;
     else if (k == "update_grid") *value = h->update_grid;

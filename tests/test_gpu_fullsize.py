@@ -66,6 +66,7 @@ def test_fullsize_per_kernel_parity(oracle_mod, cg_mod, torch_mod, full):
         h.setup(t(c["rowptr"]), t(c["colidx"]), t(c["vals"]), s)
         assert h.get_info("spmv_bulk") == 1 and h.get_info("lanes") == 1      # the configuration bench.py times
         assert h.get_info("spmv_grid") % h.get_info("num_sms") == 0
+        assert h.get_info("gram_staged") == 1 and h.get_info("block_staged") == 0   # s = 4 at 32.8 M rows: TMA-staged Gram, register update
         # a1: the MPK on the oracle's residual of iteration 3 (every element of every column)
         R, AR = h.test_mpk(t(S["r"]))
         R, AR = R.cpu().numpy(), AR.cpu().numpy()

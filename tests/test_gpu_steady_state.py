@@ -43,7 +43,7 @@ def dev(torch, a):
 
 def assert_steady_state(h, kind, n):
     """>= 2 grid-stride passes per thread (register kernels) / > 2 D tiles per CTA (staged kernels)."""
-    if h.get_info("block_staged"):
+    if h.get_info("gram_staged" if kind == "gram" else "block_staged"):
         T, D, grid = h.get_info(f"{kind}_tile_rows"), h.get_info(f"{kind}_ring_depth"), h.get_info(f"{kind}_grid")
         tiles_per_cta = ((n + T - 1) // T) // grid
         assert T > 0 and D > 0 and tiles_per_cta > 2 * D, (kind, T, D, grid, tiles_per_cta)
@@ -58,10 +58,15 @@ def gram_close(M, Mr, A, B):
 
 
 @pytest.mark.parametrize("s", S_ALL)
-@pytest.mark.parametrize("block_variant", [0, 1])
+@pytest.mark.parametrize("block_variant", [0, 1, 2])
 def test_gram_parity_steady_state(oracle_mod, cg_mod, torch_mod, big_1d, s, block_variant):
+    """block_variant 0: the solver's choice at this size (register kernel for s <= 4, TMA-staged above); 1: the register
+    kernel forced (three block sizes above s = 4); 2: the TMA-staged kernel forced for s <= 4 -- the solver's choice for
+    s = 2..4 from 3 M rows on, i.e. on the headline workload (tiles of 512 rows, at most 32 bulk copies in flight per SM)."""
     if block_variant == 1 and s not in (5, 8, 16):
         pytest.skip("the register kernels are the default below s = 5; forced above only for three block sizes")
+    if block_variant == 2 and s > 4:
+        pytest.skip("the staged kernel is already the default from s = 5 on")
     n = N_BIG
     rng = np.random.default_rng(1100 + s)
     R, AR, AP = (rng.uniform(-1, 1, (s, n)) for _ in range(3))
@@ -69,7 +74,7 @@ def test_gram_parity_steady_state(oracle_mod, cg_mod, torch_mod, big_1d, s, bloc
     rp, ci, v = big_1d
     with cg_mod.SStepCG(0, block_variant=block_variant) as h:
         h.setup(dev(torch_mod, rp), dev(torch_mod, ci), dev(torch_mod, v), s)
-        assert h.get_info("block_staged") == (1 if (s >= 5 and block_variant == 0) else 0)
+        assert h.get_info("gram_staged") == (1 if (block_variant == 2 or (s >= 5 and block_variant == 0)) else 0)
         assert_steady_state(h, "gram", n)
         M, C, m = (t.cpu().numpy() for t in h.test_gram(*(dev(torch_mod, a) for a in (R, AR, AP, r))))
     Mr, Cr, mr = oracle_mod.gram(R, AR, AP, r)
