@@ -32,13 +32,15 @@ import sstep_inputs as gen  # noqa: E402
 NS = 2048            # sampled entries of x per fixture
 SAMPLE_SEED = 777    # numpy.random.default_rng(SAMPLE_SEED).choice(n, NS, replace=False), sorted
 
-# case -> (config, s, basis, method); method "sstep" = Alg. 3, "pcg" = Alg. 1, "pfcg" = Alg. 2
+# case -> (config, s, basis, method); method "sstep" = Alg. 3 (Gram form), "sstep_moment" = Alg. 3 with Alg. 5 + 6, "pcg" = Alg. 1
 CASES = {
     "config1_s2": (1, 2, 0, "sstep"), "config2_s4": (2, 4, 0, "sstep"), "config3_s4": (3, 4, 0, "sstep"),
     "config4_s1": (4, 1, 0, "sstep"), "config4_s2": (4, 2, 0, "sstep"), "config4_s4": (4, 4, 0, "sstep"),
     "config5_s8_cheb": (5, 8, 1, "sstep"), "config5_s8_mono": (5, 8, 0, "sstep"),
     "config6_s1": (6, 1, 0, "sstep"), "config6_s2": (6, 2, 0, "sstep"), "config6_s3": (6, 3, 0, "sstep"),
     "config6_s4": (6, 4, 0, "sstep"), "config6_s5": (6, 5, 0, "sstep"), "config6_pcg": (6, 1, 0, "pcg"),
+    # the paper-literal moment form (Alg. 5 + Alg. 6 with the moments taken in the SpMV epilogues: oracle form "moment_fused")
+    "config4_s4_moment": (4, 4, 0, "sstep_moment"), "config6_s4_moment": (6, 4, 0, "sstep_moment"),
 }
 
 
@@ -54,13 +56,13 @@ def run_case(name: str, N: int | None = None) -> str:
         ref = oracle.pcg(c["rowptr"], c["colidx"], c["vals"], c["b"], rtol=c["rtol"], maxit=c["maxit"], history=True)
     else:
         ref = oracle.sstep(c["rowptr"], c["colidx"], c["vals"], c["b"], s, rtol=c["rtol"], maxit=c["maxit"], basis=basis,
-                           history=True)
+                           history=True, form="moment_fused" if method == "sstep_moment" else "gram")
     dt = time.time() - t0
     x = ref["x"]
     idx = sample_indices(c["n"])
     lines = [
         f"# tests/golden/{name}.txt -- written by `python tests/golden/make_golden.py --case {name}" + (f" --grid {N}`" if N else "`"),
-        "# from oracle/ only (oracle.pcg = Alg. 1, PAPER.md:48-73; oracle.sstep = Alg. 3, PAPER.md:158, Gram form; stop test",
+        "# from oracle/ only (oracle.pcg = Alg. 1, PAPER.md:48-73; oracle.sstep = Alg. 3, PAPER.md:158, Gram or moment form; stop test",
         "# ||r||_2 < rtol ||r_0||_2, PAPER.md:259).  Never edited by hand, never written from the CUDA path.",
         f"# workload: sstep_inputs.make_config({cfg}" + (f", N={N}" if N else "") + f") = {c['name']}, n = {c['n']}, nnz = {c['nnz']}, rtol = {c['rtol']:g}",
         f"# oracle wall time {dt:.0f} s (one thread)",

@@ -166,6 +166,15 @@ def test_config4_solve_host_matches_golden(oracle_mod, cg_mod, torch_mod):
             assert np.all(np.isfinite(xh))
 
 
+@pytest.mark.parametrize("name", ["config6_s4_moment", "config4_s4_moment"])
+def test_moment_form_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod, name):
+    """The paper-literal form (Alg. 5 + Alg. 6; option form = 1: the 2s moments accumulated in the SpMV
+    epilogues, no Gram pass -- the `moment_form` lines of bench.py) at full size against fixtures the oracle wrote in ITS
+    moment form (orc_sstep, form "moment_fused"): the paper's 250^3 problem and the headline 320^3 workload, whole solves."""
+    res = check_against_golden(oracle_mod, cg_mod, torch_mod, name, x_tol=1e-8, hist_tol=1e-4, form=1)
+    assert res["status"] == 0
+
+
 def test_config5_chebyshev_converged_solve_matches_golden(oracle_mod, cg_mod, torch_mod):
     """Config 5 (256^3 variable coefficients, permuted rows -> auto-reordered, s = 8) with the Chebyshev basis."""
     check_against_golden(oracle_mod, cg_mod, torch_mod, "config5_s8_cheb", x_tol=1e-8, hist_tol=1e-6)
