@@ -21,7 +21,7 @@ struct GramTmaCfg {
     static constexpr int NACC = 2 * S * G + G;
     static constexpr int RPP = 32 / NSL;                                         // rows per warp pass
     static constexpr int NWC = 8;                                                // consumer warps
-    static constexpr int T = (S <= 4) ? 512 : (S <= 8) ? 128 : 64;               // rows per tile
+    static constexpr int T = (S <= 4) ? 512 : (S == 5) ? 384 : (S <= 8) ? 128 : 64;   // rows per tile (s <= 5: few large copies in flight)
     static constexpr int PASSES = T / (NWC * RPP);
     static constexpr int COLS = T + 2;                                           // column slice + alignment slack
     static constexpr int OFF_AR = S * COLS, OFF_AP = 2 * S * COLS, OFF_r = OFF_AP + T * S + 2;
@@ -29,7 +29,7 @@ struct GramTmaCfg {
     static constexpr int D_FIT = ((S <= 8 ? 192 : 144) * 1024) / (SLOT * 8);  // one CTA per SM: the ring takes most of its shared memory
     static constexpr int D = D_FIT > 8 ? 8 : (D_FIT < 2 ? 2 : D_FIT);
     static constexpr int NSEG = 2 * S + 2;
-    static constexpr int NPW = (S <= 4) ? 3 : 4;                  // producer warps (tile i is filled by warp i % NPW)
+    static constexpr int NPW = (S <= 5) ? 3 : 4;                  // producer warps (tile i is filled by warp i % NPW)
     static constexpr int THREADS = (NWC + NPW) * 32;
     static constexpr size_t SMEM = (size_t)D * SLOT * sizeof(double) + 2 * D * sizeof(uint64_t);
     static_assert(PASSES >= 1 && T % (NWC * RPP) == 0, "tile must hold whole passes of all consumer warps");
